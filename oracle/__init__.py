@@ -1,0 +1,113 @@
+"""ctypes front end of the CPU oracle (gp_oracle.c).  TEST INFRASTRUCTURE ONLY.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference
+legs may import this package.  It imports nothing from the CUDA path.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from concurrent.futures import ThreadPoolExecutor
+
+import numpy as np
+
+from .build import build as _build
+
+_PRIM_BYTES = 48
+
+
+class Params(ctypes.Structure):
+    _fields_ = [("cam_height", ctypes.c_float), ("t_max", ctypes.c_float),
+                ("fov_rad", ctypes.c_float), ("ambient", ctypes.c_float),
+                ("light", ctypes.c_float * 3), ("palette", (ctypes.c_uint8 * 3) * 4)]
+
+
+def make_params(cam_height=1.6, t_max=100.0, fov_rad=np.float32(np.pi / 2), ambient=0.25,
+                light=(0.48, 0.36, 0.8),
+                palette=((135, 206, 235), (90, 90, 90), (240, 240, 240), (40, 80, 220))) -> Params:
+    p = Params()
+    p.cam_height, p.t_max, p.fov_rad, p.ambient = cam_height, t_max, float(fov_rad), ambient
+    for i in range(3):
+        p.light[i] = light[i]
+    for c in range(4):
+        for ch in range(3):
+            p.palette[c][ch] = int(palette[c][ch])
+    return p
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        L = ctypes.CDLL(_build())
+        vp, ci, cf = ctypes.c_void_p, ctypes.c_int, ctypes.c_float
+        L.orc_render_view.argtypes = [vp, ci, ci, cf, cf, ctypes.POINTER(Params), ci, ci,
+                                      vp, vp, vp, vp, vp, vp]
+        L.orc_render_view.restype = ci
+        L.orc_shadow_view.argtypes = [vp, ci, ci, cf, cf, ctypes.POINTER(Params), ci, ci,
+                                      vp, vp, vp, vp]
+        L.orc_shadow_view.restype = ci
+        _lib = L
+    return _lib
+
+
+def _check_prims(prims):
+    prims = np.ascontiguousarray(prims)
+    assert prims.dtype.itemsize == _PRIM_BYTES and prims.ndim == 1, (prims.dtype, prims.shape)
+    return prims
+
+
+def render_view(prims, ego, H, W, params=None, cp=1.0, sp=0.0, rgb=True):
+    """fp32-contract render of one view.  prims: 1-D structured array (48-byte records) of the
+    ego's world.  Returns dict(cls u8[H,W], inst i32[H,W], depth f32[H,W], rgb u8[3,H,W] or None,
+    t2 f32[H,W], win i32[H,W])."""
+    prims = _check_prims(prims)
+    params = params or make_params()
+    out = {"cls": np.empty((H, W), np.uint8), "inst": np.empty((H, W), np.int32),
+           "depth": np.empty((H, W), np.float32),
+           "rgb": np.empty((3, H, W), np.uint8) if rgb else None,
+           "t2": np.empty((H, W), np.float32), "win": np.empty((H, W), np.int32)}
+    rc = lib().orc_render_view(prims.ctypes.data, len(prims), int(ego), float(cp), float(sp),
+                               ctypes.byref(params), H, W,
+                               out["cls"].ctypes.data, out["inst"].ctypes.data, out["depth"].ctypes.data,
+                               out["rgb"].ctypes.data if rgb else None,
+                               out["t2"].ctypes.data, out["win"].ctypes.data)
+    if rc != 0:
+        raise ValueError("orc_render_view: bad arguments")
+    return out
+
+
+def shadow_view(prims, ego, H, W, params=None, cp=1.0, sp=0.0):
+    """fp64 face-enumeration render of one view: dict(win i32, depth f64, t2 f64, ndl f64)."""
+    prims = _check_prims(prims)
+    params = params or make_params()
+    out = {"win": np.empty((H, W), np.int32), "depth": np.empty((H, W), np.float64),
+           "t2": np.empty((H, W), np.float64), "ndl": np.empty((H, W), np.float64)}
+    rc = lib().orc_shadow_view(prims.ctypes.data, len(prims), int(ego), float(cp), float(sp),
+                               ctypes.byref(params), H, W, out["win"].ctypes.data,
+                               out["depth"].ctypes.data, out["t2"].ctypes.data, out["ndl"].ctypes.data)
+    if rc != 0:
+        raise ValueError("orc_shadow_view: bad arguments")
+    return out
+
+
+def render_views(world_prims, views, H, W, params=None, pitch_cs=None, rgb=True, threads=1,
+                 shadow=False):
+    """Render a list of (world, agent) views.  world_prims: [Wn][P] structured array.  The
+    renderer itself is single-threaded; `threads` > 1 runs the same code over disjoint views
+    (ctypes releases the GIL).  Returns a list of dicts in the order of `views`."""
+    params = params or make_params()
+
+    def one(wa):
+        w, a = wa
+        cp, sp = (1.0, 0.0) if pitch_cs is None else (float(pitch_cs[w, a, 0]), float(pitch_cs[w, a, 1]))
+        fn = shadow_view if shadow else render_view
+        kw = {} if shadow else {"rgb": rgb}
+        return fn(world_prims[w], a, H, W, params, cp, sp, **kw)
+
+    if threads <= 1:
+        return [one(v) for v in views]
+    with ThreadPoolExecutor(max_workers=threads) as ex:
+        return list(ex.map(one, views))
