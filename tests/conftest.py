@@ -1,0 +1,45 @@
+import os
+import sys
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+
+def pytest_configure(config):
+    config.addinivalue_line("markers", "gpu: needs a B200 (run with -m gpu on the GPU box)")
+
+
+import gp_scenes as gs  # noqa: E402
+
+
+def make_prim(cx, cy, cz, hx, hy, hz, cos_yaw=1.0, sin_yaw=0.0, cls=3, inst=0):
+    p = np.zeros((), dtype=gs.PRIM_DTYPE)
+    p["cx"], p["cy"], p["cz"] = cx, cy, cz
+    p["hx"], p["hy"], p["hz"] = hx, hy, hz
+    p["cos_yaw"], p["sin_yaw"] = cos_yaw, sin_yaw
+    p["cls"], p["inst"] = cls, inst
+    return p
+
+
+def ego_at_origin(cos_yaw=1.0, sin_yaw=0.0, half_len=2.0):
+    """Vehicle whose front-centre (the camera foot point) is exactly the world origin."""
+    return make_prim(-half_len * cos_yaw, -half_len * sin_yaw, 0.75, half_len, 0.9, 0.75,
+                     cos_yaw, sin_yaw, cls=3, inst=0)
+
+
+def stack(*prims):
+    out = np.zeros(len(prims), dtype=gs.PRIM_DTYPE)
+    for i, p in enumerate(prims):
+        out[i] = p
+    return out
+
+
+@pytest.fixture(scope="session")
+def tiny_world():
+    cfg = gs.config("tiny")
+    a, q = gs.gen_world_prims(cfg)
+    return cfg, np.concatenate([a, q], axis=1)
