@@ -1,0 +1,148 @@
+/* gp.h — C ABI of the B200-native batched per-agent perspective renderer ("Gigapixel" hot path).
+ *
+ * What the library computes: O_pixel(S_t, i) of PAPER.md:60-62 (§3.1) — the simulator state
+ * S_t = (A_t, M, L_t) rendered into the ego-centric perspective view of every agent i of every
+ * parallel world, "thousands of environments ... in a single batched launch",
+ * cuboids for agents, planar strips for road segments, one directional light, per-instance
+ * attributes, images "exposed directly as a batched GPU tensor ... no per-step
+ * CPU transfer" with configurable resolution and camera.  The per-pixel arithmetic
+ * is the written contract C0-C8 of DESIGN.md §3 (the paper gives no formula).
+ *
+ * Conventions
+ *  - Every function returns an int status: GP_OK (0) or a negative GP_ERR_* code.  Argument errors
+ *    write nothing.  gp_error_string(code) returns a static string; after GP_ERR_CUDA it contains
+ *    the CUDA error text of the calling thread's last failure.
+ *  - "DEVICE" pointers are CUDA device pointers on the context's device; "HOST" pointers are plain
+ *    host memory.  The library never frees or keeps caller memory.  Output buffers are caller-owned.
+ *  - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Calls enqueue
+ *    work on it and return without synchronising, except where stated.
+ *  - Only sm_100 (B200) devices are accepted; there is no fallback path of any kind.
+ *  - Views are ordered world-major, then agent: view = world * agents_per_world + agent.
+ */
+#ifndef GP_H_
+#define GP_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum {
+    GP_OK = 0,
+    GP_ERR_ARG = -1,        /* NULL / non-positive / inconsistent argument                   */
+    GP_ERR_ALIGN = -2,      /* an output or input pointer is not 16-byte aligned             */
+    GP_ERR_STATE = -3,      /* call order: render / update before gp_scene_upload            */
+    GP_ERR_RANGE = -4,      /* world range outside the scene, agents != agents_per_world     */
+    GP_ERR_CUDA = -5,       /* a CUDA runtime call failed (text via gp_error_string)         */
+    GP_ERR_ARCH = -6,       /* the device is not compute capability 10.x                     */
+    GP_ERR_NOMEM = -7       /* device or host allocation failed                              */
+};
+
+/* gp_set_option keys */
+enum {
+    GP_OPT_PATH = 1,        /* GP_PATH_FAST (default) or GP_PATH_BRUTE                        */
+    GP_OPT_STATS = 2,       /* 1: count executed ray/primitive tests and listed pairs         */
+    GP_OPT_TIMING = 3       /* 1: bracket every kernel launch with CUDA events (gp_kernel_time) */
+};
+enum {                      /* kernel ids of gp_kernel_time                                   */
+    GP_KERNEL_UPDATE = 0,   /* a0 pose update + shading table                                 */
+    GP_KERNEL_CULL = 1,     /* a1 camera setup + a2 frustum cull and compaction               */
+    GP_KERNEL_RENDER = 2,   /* a3-a9 render pass (fast path)                                  */
+    GP_KERNEL_BRUTE = 3     /* brute-force kernel                                             */
+};
+enum {
+    GP_PATH_FAST = 0,       /* cull + compaction, list staged in shared memory, strip render  */
+    GP_PATH_BRUTE = 1       /* one thread per pixel, every primitive of the world, no culling */
+};
+
+typedef struct gp_ctx gp_ctx;   /* opaque, library-owned */
+
+/* Scene-wide constants (C1, C2, C4, C8).  Plain data, copied at upload. */
+typedef struct {
+    int32_t n_worlds;           /* Wn >= 1                                                    */
+    int32_t agents_per_world;   /* A >= 1: primitives 0..A-1 of a world are the agents        */
+    int32_t quads_per_world;    /* Q >= 0: primitives A..A+Q-1 are static                     */
+    float cam_height;           /* camera z, metres (1.6)                                     */
+    float t_max;                /* far plane on planar depth, metres (100); +inf allowed      */
+    float light[3];             /* unit vector towards the light (0.48, 0.36, 0.8)            */
+    float ambient;              /* in [0,1] (0.25)                                            */
+    uint8_t palette[4][3];      /* RGB of class 0 sky, 1 ground, 2 marking, 3 vehicle         */
+} gp_scene_desc;
+
+/* One primitive: an oriented box; hz == 0 makes it a flat quad (C1).  48 bytes. */
+typedef struct {
+    float cx, cy, cz;           /* centre, world frame: z up                                  */
+    float hx, hy, hz;           /* half extents along the box axes, >= 0                      */
+    float cos_yaw, sin_yaw;     /* heading of the box x axis                                  */
+    int32_t cls;                /* class id written to the class plane (0..3)                 */
+    int32_t inst;               /* instance id written to the instance plane                  */
+    int32_t pad[2];
+} gp_prim;
+
+/* Create a context on CUDA device `cuda_device`.  GP_ERR_ARCH unless it is sm_100. */
+int gp_create(gp_ctx **out, int cuda_device);
+
+/* Free every device allocation of the context.  Synchronises the device. */
+int gp_destroy(gp_ctx *ctx);
+
+int gp_set_option(gp_ctx *ctx, int key, int value);
+
+/* Step a0 (scene residency).  Copies desc, h_agents [Wn][A] and h_quads [Wn][Q] (HOST; h_quads may be
+ * NULL iff Q == 0) into library-owned device memory as one table [Wn][A+Q], derives the per-primitive
+ * shading table (C8) on the device and resets every camera pitch to 0.  The host arrays are copied
+ * into a library-owned staging buffer before the call returns, so they may be freed at once.
+ * (Re)allocates device memory: not for use inside a timed loop. */
+int gp_scene_upload(gp_ctx *ctx, const gp_scene_desc *desc, const gp_prim *h_agents,
+                    const gp_prim *h_quads, void *stream);
+
+/* Step a0 (pose update).  d_pose: DEVICE [Wn][A][4] fp32 = (cx, cy, cos yaw, sin yaw) of every agent;
+ * overwrites those four fields of the agent records and refreshes their shading table.  16-byte
+ * aligned.  No host transfer. */
+int gp_agents_update(gp_ctx *ctx, const float *d_pose, void *stream);
+
+/* Camera pitch per view.  d_pitch_cs: DEVICE [Wn][A][2] fp32 = (cos p, sin p), positive = nose up;
+ * NULL resets every camera to pitch 0.  Copied on `stream`. */
+int gp_cameras_set(gp_ctx *ctx, const float *d_pitch_cs, void *stream);
+
+/* Steps a1-a9.  Renders the views of worlds [world_begin, world_begin + n_worlds) at H x W pixels with
+ * horizontal field of view fov_rad (vertical follows from square pixels).  `agents` must equal
+ * agents_per_world.  Outputs (DEVICE, 16-byte aligned, n = n_worlds*agents views, row-major, row 0 = top):
+ *   d_class    [n][H][W]    uint8   0 sky, 1 ground, else the winning primitive's cls
+ *   d_instance [n][H][W]    int32   the winning primitive's inst; -1 for ground and sky
+ *   d_depth    [n][H][W]    float   planar depth of the nearest hit; 0 for sky
+ *   d_rgb      [n][3][H][W] uint8   shaded colour, planar; NULL skips the plane
+ * 1 <= H, W <= 4096.  The fast path needs W % 4 == 0; other widths take the brute-force path.
+ * May grow library-owned scratch on first use of a larger (n_worlds, H, W): warm up before timing. */
+int gp_render_batch(gp_ctx *ctx, int world_begin, int n_worlds, int agents, int H, int W,
+                    float fov_rad, uint8_t *d_class, int32_t *d_instance, float *d_depth,
+                    uint8_t *d_rgb, void *stream);
+
+/* End-to-end variant with HOST buffers: copies h_pose (HOST [Wn][A][4], may be NULL = keep poses) to the
+ * device, updates the agents, renders worlds [world_begin, world_begin+n_worlds) in chunks through
+ * library-owned device staging and copies the four planes (same layouts as above; h_rgb may be NULL)
+ * back to the HOST buffers.  Synchronises `stream` before returning.  Pinned host memory is faster
+ * but not required. */
+int gp_render_batch_host(gp_ctx *ctx, const float *h_pose, int world_begin, int n_worlds, int agents,
+                         int H, int W, float fov_rad, uint8_t *h_class, int32_t *h_instance,
+                         float *h_depth, uint8_t *h_rgb, void *stream);
+
+/* Counters of the last gp_render_batch issued with GP_OPT_STATS = 1 (synchronises the device):
+ * executed_tests = ray/primitive slab tests actually evaluated, listed_pairs = (view, primitive)
+ * pairs that survived the cull.  Either pointer may be NULL. */
+int gp_stats(gp_ctx *ctx, uint64_t *executed_tests, uint64_t *listed_pairs);
+
+/* With GP_OPT_TIMING = 1 every launch of the library is bracketed by CUDA events on the launch
+ * stream.  Returns the summed device time (milliseconds) and the number of launches of `kernel`
+ * recorded since the last call for that kernel, then forgets them.  Synchronises the device. */
+int gp_kernel_time(gp_ctx *ctx, int kernel, double *total_ms, uint64_t *launches);
+
+/* Number of kernel launches the library has issued on this context since creation. */
+int gp_launch_count(gp_ctx *ctx, uint64_t *launches);
+
+const char *gp_error_string(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GP_H_ */

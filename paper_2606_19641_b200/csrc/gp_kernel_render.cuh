@@ -1,0 +1,234 @@
+// gp_kernel_render.cuh — a3-a9: the render pass (one CTA per view).
+//
+//   prologue  one thread arms an mbarrier and issues two TMA bulk copies (cp.async.bulk, global ->
+//             shared) of the view's list (EntryGeo n*48 B, EntryAux n*16 B); meanwhile all threads
+//             build the per-column table s_j and the per-row table (v_i, d.z, 1/d.z, t_ground).
+//   strips    each warp owns strips of SR consecutive rows.  It scans the list 32 entries at a time
+//             (ballot on row overlap: the warp-level early-out), and for every overlapping entry
+//             spreads its lanes over the entry's pixel rectangle inside the strip, runs the contract
+//             slab test (C5) and keeps the lexicographic minimum (C6) as a packed 64-bit key in a
+//             shared-memory key buffer that only this warp touches (no atomics).
+//   resolve   per 4 consecutive pixels of a row: ground / sky default from the row table, patched by
+//             the key where a primitive won; shade (C8); 4-byte / 16-byte coalesced stores: a warp
+//             writes 128 consecutive pixels of every plane (full 128-byte lines).
+#pragma once
+#include "gp_device.cuh"
+
+namespace gp {
+
+struct RenderArgs {
+    const ViewHdr *hdr; const EntryGeo *geo; const EntryAux *aux; const PrimMeta *meta;
+    int cap, world_begin, H, W;
+    float th, tv;
+    int SR, log2LC;                 // rows per strip; lanes per row of the test tile (LC = 1 << log2LC)
+    uint8_t *o_cls; int32_t *o_inst; float *o_depth; uint8_t *o_rgb;
+    unsigned long long *stats;
+};
+
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t *bar, int count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
+    asm volatile(
+        "{\n .reg .pred p;\n WAIT_%=:\n"
+        " mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        " @p bra DONE_%=;\n bra WAIT_%=;\n DONE_%=:\n}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t bytes, uint64_t *bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+
+constexpr unsigned long long kKeyEmpty = 0xFFFFFFFFFFFFFFFFull;
+
+template <bool STATS>
+__global__ void __launch_bounds__(256)
+k_render(SceneConst sc, RenderArgs ra) {
+    extern __shared__ __align__(16) unsigned char smem[];
+    const int view = blockIdx.x;
+    const int H = ra.H, W = ra.W, SR = ra.SR;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
+
+    // ---- shared memory carve-up ---------------------------------------------------------------
+    uint64_t *bar = reinterpret_cast<uint64_t *>(smem);
+    EntryGeo *s_geo = reinterpret_cast<EntryGeo *>(smem + 16);
+    EntryAux *s_aux = reinterpret_cast<EntryAux *>(smem + 16 + (size_t)ra.cap * 48);
+    float4 *s_row = reinterpret_cast<float4 *>(smem + 16 + (size_t)ra.cap * 64);
+    float *s_col = reinterpret_cast<float *>(s_row + H);
+    unsigned long long *s_keys = reinterpret_cast<unsigned long long *>(s_col + ((W + 3) & ~3));
+    unsigned long long *keys = s_keys + (size_t)warp * SR * W;
+
+    const float4 vh4 = __ldg(reinterpret_cast<const float4 *>(&ra.hdr[view]));
+    ViewHdr vh; vh.n = __float_as_int(vh4.x); vh.oz = vh4.y; vh.cp = vh4.z; vh.sp = vh4.w;
+    const int n = vh.n;
+    if (threadIdx.x == 0) {
+        mbar_init(bar, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        if (n > 0) {
+            mbar_expect_tx(bar, (uint32_t)n * 64u);
+            bulk_g2s(s_geo, ra.geo + (size_t)view * ra.cap, (uint32_t)n * 48u, bar);
+            bulk_g2s(s_aux, ra.aux + (size_t)view * ra.cap, (uint32_t)n * 16u, bar);
+        }
+    }
+    // tables (contract C2-C4), overlapped with the bulk copies
+    for (int j = threadIdx.x; j < W; j += blockDim.x) s_col[j] = pix_s(j, W, ra.th);
+    for (int i = threadIdx.x; i < H; i += blockDim.x) {
+        const float v = pix_v(i, H, ra.tv);
+        const float dz = c_fma(v, vh.cp, vh.sp);
+        const float inv_z = c_rcp(dz);
+        float tg = -1.0f;
+        if (dz < 0.0f) {
+            const float t = c_mul(c_sub(0.0f, vh.oz), inv_z);
+            if (t > 0.0f && t <= sc.t_max) tg = t;
+        }
+        s_row[i] = make_float4(v, dz, inv_z, tg);
+    }
+    __syncthreads();                       // tables + mbarrier init visible
+    if (n > 0) mbar_wait(bar, 0);
+
+    const int w = ra.world_begin + view / sc.A;
+    const PrimMeta *wmeta = ra.meta + (size_t)w * sc.P;
+    const int s8_ground = shade_scale(c_max(sc.Lz, 0.0f), sc.ambient);
+    const uint32_t rgb_ground = shade_rgb(sc.pal[1], s8_ground), rgb_sky = sc.pal[0];
+    const int LC = 1 << ra.log2LC, LR = 32 >> ra.log2LC;
+    const int li = lane >> ra.log2LC, lj = lane & (LC - 1);
+    const size_t HW = (size_t)H * W;
+    const int n_strips = (H + SR - 1) / SR;
+    unsigned long long n_tests = 0;
+
+    for (int strip = warp; strip < n_strips; strip += nwarps) {
+        const int row0 = strip * SR, row1 = min(H, row0 + SR) - 1;
+        bool any = false;
+        // ---- a3: warp-level early-out over the list, a6/a7: slab test + select ----------------
+        for (int base = 0; base < n; base += 32) {
+            const int e = base + lane;
+            bool ov = false;
+            if (e < n) {
+                const uint32_t rows = s_aux[e].rows;
+                ov = (int)(rows & 0xffff) <= row1 && (int)(rows >> 16) >= row0;
+            }
+            unsigned mask = __ballot_sync(0xffffffffu, ov);
+            if (mask && !any) {
+                any = true;
+                ulonglong2 *k2 = reinterpret_cast<ulonglong2 *>(keys);
+                const int nk2 = (row1 - row0 + 1) * W / 2;
+                for (int q = lane; q < nk2; q += 32) k2[q] = make_ulonglong2(kKeyEmpty, kKeyEmpty);
+                __syncwarp();
+            }
+            while (mask) {
+                const int eb = base + __ffs(mask) - 1;
+                mask &= mask - 1;
+                const float4 g0 = *reinterpret_cast<const float4 *>(&s_geo[eb]);
+                const float4 g1 = *(reinterpret_cast<const float4 *>(&s_geo[eb]) + 1);
+                const float4 g2 = *(reinterpret_cast<const float4 *>(&s_geo[eb]) + 2);
+                const uint4 ax = *reinterpret_cast<const uint4 *>(&s_aux[eb]);
+                const bool flat = ax.x & 1u;
+                const uint32_t klow = (ax.x >> 1) << 3;
+                const int r0 = max((int)(ax.y & 0xffff), row0), r1 = min((int)(ax.y >> 16), row1);
+                const int c0 = (int)(ax.z & 0xffff), c1 = (int)(ax.z >> 16);
+                for (int rb = r0; rb <= r1; rb += LR) {
+                    const int i = rb + li;
+                    for (int cb = c0; cb <= c1; cb += LC) {
+                        const int j = cb + lj;
+                        if (i <= r1 && j <= c1) {
+                            if (STATS) ++n_tests;
+                            const float s = s_col[j];
+                            const float4 rt = s_row[i];                     // v, dz, 1/dz, tg
+                            // C5, per-pixel part
+                            const float dlx = c_fma(rt.x, g2.z, c_fma(s, g2.x, g1.z));
+                            const float dly = c_fma(rt.x, g2.w, c_fma(s, g2.y, g1.w));
+                            const float ix = c_rcp(dlx), iy = c_rcp(dly);
+                            float ta, tb;
+                            ta = c_mul(g0.x, ix); tb = c_mul(g0.y, ix);
+                            const float lox = c_min(ta, tb), hix = c_max(ta, tb);
+                            ta = c_mul(g0.z, iy); tb = c_mul(g0.w, iy);
+                            const float loy = c_min(ta, tb), hiy = c_max(ta, tb);
+                            ta = c_mul(g1.x, rt.z); tb = c_mul(g1.y, rt.z);
+                            const float loz = c_min(ta, tb), hiz = c_max(ta, tb);
+                            const float tn = c_max(c_max(lox, loy), loz);
+                            const float tf = c_min(c_min(hix, hiy), hiz);
+                            if (tn <= tf && tn > 0.0f && tn <= sc.t_max) {
+                                uint32_t face;                                  // m*2 + (sigma > 0)
+                                if (flat) face = 5;
+                                else if (lox == tn) face = 0 + (dlx > 0.0f ? 0 : 1);
+                                else if (loy == tn) face = 2 + (dly > 0.0f ? 0 : 1);
+                                else face = 4 + (rt.y > 0.0f ? 0 : 1);
+                                const unsigned long long key =
+                                    ((unsigned long long)__float_as_uint(tn) << 32) | klow | face;   // C6
+                                unsigned long long *kp = &keys[(i - row0) * W + j];
+                                if (key < *kp) *kp = key;
+                            }
+                        }
+                    }
+                }
+                __syncwarp();
+            }
+        }
+        // ---- a5 ground, a7 resolve, a8 shade, a9 store: 4 consecutive pixels per lane ----------
+        const int nquads = (row1 - row0 + 1) * W / 4;
+        const size_t vbase = (size_t)view * HW + (size_t)row0 * W;
+        for (int q = lane; q < nquads; q += 32) {
+            const int p = q * 4;
+            const int i = row0 + p / W;
+            const float tg = s_row[i].w;
+            const bool ground = tg > 0.0f;
+            uint32_t cls4 = ground ? 0x01010101u : 0u;
+            int4 inst4 = make_int4(-1, -1, -1, -1);
+            const float d0 = ground ? tg : 0.0f;
+            float4 dep4 = make_float4(d0, d0, d0, d0);
+            const uint32_t bg = ground ? rgb_ground : rgb_sky;
+            uint32_t r4 = (bg & 0xff) * 0x01010101u, g4 = ((bg >> 8) & 0xff) * 0x01010101u,
+                     b4 = ((bg >> 16) & 0xff) * 0x01010101u;
+            if (any) {
+                const ulonglong2 ka = *reinterpret_cast<const ulonglong2 *>(&keys[p]);
+                const ulonglong2 kb = *reinterpret_cast<const ulonglong2 *>(&keys[p + 2]);
+                const unsigned long long kk[4] = {ka.x, ka.y, kb.x, kb.y};
+                if ((ka.x & ka.y & kb.x & kb.y) != kKeyEmpty) {
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) {
+                        if (kk[u] == kKeyEmpty) continue;
+                        const float t = __uint_as_float((uint32_t)(kk[u] >> 32));
+                        if (ground && !(t <= tg)) continue;                // the ground is nearer (C6)
+                        const uint32_t lo = (uint32_t)kk[u];
+                        const uint4 m = __ldg(reinterpret_cast<const uint4 *>(&wmeta[lo >> 3]));
+                        const uint32_t face = lo & 7u;
+                        const uint32_t sw = face < 2 ? m.y : face < 4 ? m.z : m.w;
+                        const int s8 = (int)((face & 1u) ? (sw >> 16) : (sw & 0xffffu)) & 0x1ff;
+                        const uint32_t c = (m.y >> 12) & 0xfu;
+                        const uint32_t rgb = c == 0 ? sc.pal[0] : shade_rgb(sc.pal[c & 3], s8);
+                        const int sh = u * 8;
+                        const uint32_t keep = ~(0xffu << sh);
+                        cls4 = (cls4 & keep) | (c << sh);
+                        r4 = (r4 & keep) | ((rgb & 0xff) << sh);
+                        g4 = (g4 & keep) | (((rgb >> 8) & 0xff) << sh);
+                        b4 = (b4 & keep) | (((rgb >> 16) & 0xff) << sh);
+                        (&inst4.x)[u] = (int)m.x;
+                        (&dep4.x)[u] = t;
+                    }
+                }
+            }
+            const size_t o = vbase + p;
+            *reinterpret_cast<uint32_t *>(ra.o_cls + o) = cls4;
+            *reinterpret_cast<int4 *>(ra.o_inst + o) = inst4;
+            *reinterpret_cast<float4 *>(ra.o_depth + o) = dep4;
+            if (ra.o_rgb) {
+                uint8_t *rb = ra.o_rgb + (size_t)view * 3 * HW + (size_t)row0 * W + p;
+                *reinterpret_cast<uint32_t *>(rb) = r4;
+                *reinterpret_cast<uint32_t *>(rb + HW) = g4;
+                *reinterpret_cast<uint32_t *>(rb + 2 * HW) = b4;
+            }
+        }
+        __syncwarp();      // the key buffer is reused by this warp's next strip
+    }
+    if (STATS) {
+        for (int o = 16; o; o >>= 1) n_tests += __shfl_xor_sync(0xffffffffu, n_tests, o);
+        if (lane == 0 && ra.stats) atomicAdd(&ra.stats[0], n_tests);
+    }
+}
+
+}  // namespace gp

@@ -1,0 +1,415 @@
+// gp_lib.cu — the C ABI of include/gp.h on top of the sm_100a kernels.  Host logic only: argument
+// validation, device residency of the scene, scratch sizing, launches.  No CPU rendering path exists.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "gp_device.cuh"
+#include "gp_kernels_basic.cuh"
+#include "gp_kernel_cull.cuh"
+#include "gp_kernel_render.cuh"
+
+using namespace gp;
+
+struct gp_ctx {
+    int device = -1;
+    bool have_scene = false;
+    SceneConst sc{};
+    gp_prim *d_prims = nullptr;
+    PrimMeta *d_meta = nullptr;
+    float2 *d_pitch = nullptr;
+    gp_prim *h_stage = nullptr; size_t h_stage_bytes = 0;        // pinned upload staging
+    // per-view scratch of the fast path
+    ViewHdr *d_hdr = nullptr; EntryGeo *d_geo = nullptr; EntryAux *d_aux = nullptr;
+    size_t scratch_views = 0; int scratch_cap = 0;
+    unsigned long long *d_stats = nullptr;
+    int opt_path = GP_PATH_FAST, opt_stats = 0, opt_timing = 0;
+    struct Timed { int kernel; cudaEvent_t a, b; };
+    std::vector<Timed> timed;                                    // GP_OPT_TIMING records
+    std::vector<cudaEvent_t> ev_pool;
+    uint64_t launches = 0;
+    size_t render_smem_set = 0;
+    // gp_render_batch_host staging
+    float *d_pose = nullptr;
+    unsigned char *d_out[2] = {nullptr, nullptr}; size_t d_out_bytes = 0;
+    cudaStream_t copy_stream = nullptr; cudaEvent_t ev_render[2] = {nullptr, nullptr}, ev_copy[2] = {nullptr, nullptr};
+};
+
+static thread_local char g_cuda_msg[256] = "CUDA error";
+
+static int cuda_fail(cudaError_t e, const char *where) {
+    snprintf(g_cuda_msg, sizeof g_cuda_msg, "CUDA error at %s: %s", where, cudaGetErrorString(e));
+    return GP_ERR_CUDA;
+}
+#define CK(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cuda_fail(e_, #call); } while (0)
+
+// Brackets one kernel launch with events when GP_OPT_TIMING is on.
+struct LaunchTimer {
+    gp_ctx *c; cudaStream_t s; bool on; gp_ctx::Timed t{};
+    LaunchTimer(gp_ctx *c_, int kernel, cudaStream_t s_) : c(c_), s(s_), on(c_->opt_timing != 0) {
+        if (!on) return;
+        t.kernel = kernel;
+        cudaEvent_t *e[2] = {&t.a, &t.b};
+        for (auto p : e) {
+            if (!c->ev_pool.empty()) { *p = c->ev_pool.back(); c->ev_pool.pop_back(); }
+            else if (cudaEventCreate(p) != cudaSuccess) { on = false; return; }
+        }
+        cudaEventRecord(t.a, s);
+    }
+    ~LaunchTimer() { if (on) { cudaEventRecord(t.b, s); c->timed.push_back(t); } }
+};
+
+static bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+extern "C" const char *gp_error_string(int code) {
+    switch (code) {
+        case GP_OK: return "ok";
+        case GP_ERR_ARG: return "invalid argument";
+        case GP_ERR_ALIGN: return "pointer not 16-byte aligned";
+        case GP_ERR_STATE: return "no scene uploaded";
+        case GP_ERR_RANGE: return "world range or agent count outside the scene";
+        case GP_ERR_CUDA: return g_cuda_msg;
+        case GP_ERR_ARCH: return "device is not sm_100 (B200); no fallback path exists";
+        case GP_ERR_NOMEM: return "out of memory";
+        default: return "unknown error code";
+    }
+}
+
+extern "C" int gp_create(gp_ctx **out, int cuda_device) {
+    if (!out) return GP_ERR_ARG;
+    *out = nullptr;
+    int count = 0;
+    CK(cudaGetDeviceCount(&count));
+    if (cuda_device < 0 || cuda_device >= count) return GP_ERR_ARG;
+    cudaDeviceProp prop;
+    CK(cudaGetDeviceProperties(&prop, cuda_device));
+    if (prop.major != 10) return GP_ERR_ARCH;
+    CK(cudaSetDevice(cuda_device));
+    gp_ctx *c = new (std::nothrow) gp_ctx();
+    if (!c) return GP_ERR_NOMEM;
+    c->device = cuda_device;
+    cudaError_t e = cudaMalloc(&c->d_stats, 2 * sizeof(unsigned long long));
+    if (e != cudaSuccess) { delete c; return cuda_fail(e, "cudaMalloc(stats)"); }
+    cudaMemset(c->d_stats, 0, 2 * sizeof(unsigned long long));
+    *out = c;
+    return GP_OK;
+}
+
+static void free_scene(gp_ctx *c) {
+    cudaFree(c->d_prims); cudaFree(c->d_meta); cudaFree(c->d_pitch);
+    c->d_prims = nullptr; c->d_meta = nullptr; c->d_pitch = nullptr;
+    cudaFree(c->d_hdr); cudaFree(c->d_geo); cudaFree(c->d_aux);
+    c->d_hdr = nullptr; c->d_geo = nullptr; c->d_aux = nullptr; c->scratch_views = 0; c->scratch_cap = 0;
+    cudaFree(c->d_pose); c->d_pose = nullptr;
+    c->have_scene = false;
+}
+
+extern "C" int gp_destroy(gp_ctx *c) {
+    if (!c) return GP_ERR_ARG;
+    cudaSetDevice(c->device);
+    cudaDeviceSynchronize();
+    free_scene(c);
+    for (int i = 0; i < 2; ++i) {
+        cudaFree(c->d_out[i]);
+        if (c->ev_render[i]) cudaEventDestroy(c->ev_render[i]);
+        if (c->ev_copy[i]) cudaEventDestroy(c->ev_copy[i]);
+    }
+    for (auto &t : c->timed) { cudaEventDestroy(t.a); cudaEventDestroy(t.b); }
+    for (auto e : c->ev_pool) cudaEventDestroy(e);
+    if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
+    if (c->h_stage) cudaFreeHost(c->h_stage);
+    cudaFree(c->d_stats);
+    delete c;
+    return GP_OK;
+}
+
+extern "C" int gp_set_option(gp_ctx *c, int key, int value) {
+    if (!c) return GP_ERR_ARG;
+    switch (key) {
+        case GP_OPT_PATH:
+            if (value != GP_PATH_FAST && value != GP_PATH_BRUTE) return GP_ERR_ARG;
+            c->opt_path = value; return GP_OK;
+        case GP_OPT_STATS:
+            c->opt_stats = value ? 1 : 0; return GP_OK;
+        case GP_OPT_TIMING:
+            c->opt_timing = value ? 1 : 0; return GP_OK;
+        default: return GP_ERR_ARG;
+    }
+}
+
+extern "C" int gp_scene_upload(gp_ctx *c, const gp_scene_desc *d, const gp_prim *h_agents,
+                               const gp_prim *h_quads, void *stream_) {
+    if (!c || !d || !h_agents) return GP_ERR_ARG;
+    if (d->n_worlds < 1 || d->agents_per_world < 1 || d->quads_per_world < 0) return GP_ERR_ARG;
+    if (d->quads_per_world > 0 && !h_quads) return GP_ERR_ARG;
+    if (!(d->cam_height > 0.0f) || !(d->t_max > 0.0f) || !(d->ambient >= 0.0f && d->ambient <= 1.0f)) return GP_ERR_ARG;
+    const long long P = (long long)d->agents_per_world + d->quads_per_world;
+    if (P > (1 << 20) || (long long)d->n_worlds * P > (1ll << 31)) return GP_ERR_ARG;
+    const size_t Wn = d->n_worlds, A = d->agents_per_world, Q = d->quads_per_world, n = Wn * (size_t)P;
+    for (size_t i = 0; i < Wn * A; ++i) {
+        const gp_prim &p = h_agents[i];
+        if (p.cls < 0 || p.cls > 3 || !(p.hx >= 0.0f && p.hy >= 0.0f && p.hz >= 0.0f)) return GP_ERR_ARG;
+    }
+    for (size_t i = 0; i < Wn * Q; ++i) {
+        const gp_prim &p = h_quads[i];
+        if (p.cls < 0 || p.cls > 3 || !(p.hx >= 0.0f && p.hy >= 0.0f && p.hz >= 0.0f)) return GP_ERR_ARG;
+    }
+    cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+    CK(cudaSetDevice(c->device));
+    CK(cudaDeviceSynchronize());            // earlier work may still read the old scene
+    free_scene(c);
+    if (c->h_stage_bytes < n * sizeof(gp_prim)) {
+        if (c->h_stage) cudaFreeHost(c->h_stage);
+        c->h_stage = nullptr; c->h_stage_bytes = 0;
+        if (cudaMallocHost(&c->h_stage, n * sizeof(gp_prim)) != cudaSuccess) { cudaGetLastError(); return GP_ERR_NOMEM; }
+        c->h_stage_bytes = n * sizeof(gp_prim);
+    }
+    for (size_t w = 0; w < Wn; ++w) {       // interleave into one table [Wn][A+Q]
+        memcpy(c->h_stage + w * P, h_agents + w * A, A * sizeof(gp_prim));
+        if (Q) memcpy(c->h_stage + w * P + A, h_quads + w * Q, Q * sizeof(gp_prim));
+    }
+    if (cudaMalloc(&c->d_prims, n * sizeof(gp_prim)) != cudaSuccess ||
+        cudaMalloc(&c->d_meta, n * sizeof(PrimMeta)) != cudaSuccess ||
+        cudaMalloc(&c->d_pitch, Wn * A * sizeof(float2)) != cudaSuccess ||
+        cudaMalloc(&c->d_pose, Wn * A * 4 * sizeof(float)) != cudaSuccess) {
+        cudaGetLastError(); free_scene(c); return GP_ERR_NOMEM;
+    }
+    SceneConst &sc = c->sc;
+    sc.Wn = (int)Wn; sc.A = (int)A; sc.Q = (int)Q; sc.P = (int)P;
+    sc.cam_h = d->cam_height; sc.t_max = d->t_max;
+    sc.Lx = d->light[0]; sc.Ly = d->light[1]; sc.Lz = d->light[2]; sc.ambient = d->ambient;
+    for (int k = 0; k < 4; ++k)
+        sc.pal[k] = (uint32_t)d->palette[k][0] | ((uint32_t)d->palette[k][1] << 8) | ((uint32_t)d->palette[k][2] << 16);
+    CK(cudaMemcpyAsync(c->d_prims, c->h_stage, n * sizeof(gp_prim), cudaMemcpyHostToDevice, stream));
+    k_prim_meta<<<(unsigned)((n + 255) / 256), 256, 0, stream>>>(sc, c->d_prims, c->d_meta);
+    k_fill_pitch<<<(unsigned)((Wn * A + 255) / 256), 256, 0, stream>>>(c->d_pitch, Wn * A);
+    c->launches += 2;
+    CK(cudaGetLastError());
+    c->have_scene = true;
+    return GP_OK;
+}
+
+extern "C" int gp_agents_update(gp_ctx *c, const float *d_pose, void *stream_) {
+    if (!c || !d_pose) return GP_ERR_ARG;
+    if (!c->have_scene) return GP_ERR_STATE;
+    if (!aligned16(d_pose)) return GP_ERR_ALIGN;
+    const size_t n = (size_t)c->sc.Wn * c->sc.A;
+    {
+        LaunchTimer lt(c, GP_KERNEL_UPDATE, static_cast<cudaStream_t>(stream_));
+        k_agents_update<<<(unsigned)((n + 255) / 256), 256, 0, static_cast<cudaStream_t>(stream_)>>>(
+            c->sc, reinterpret_cast<const float4 *>(d_pose), c->d_prims, c->d_meta);
+    }
+    c->launches += 1;
+    CK(cudaGetLastError());
+    return GP_OK;
+}
+
+extern "C" int gp_cameras_set(gp_ctx *c, const float *d_pitch_cs, void *stream_) {
+    if (!c) return GP_ERR_ARG;
+    if (!c->have_scene) return GP_ERR_STATE;
+    const size_t n = (size_t)c->sc.Wn * c->sc.A;
+    cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+    if (d_pitch_cs) {
+        CK(cudaMemcpyAsync(c->d_pitch, d_pitch_cs, n * sizeof(float2), cudaMemcpyDeviceToDevice, stream));
+    } else {
+        k_fill_pitch<<<(unsigned)((n + 255) / 256), 256, 0, stream>>>(c->d_pitch, n);
+        c->launches += 1;
+        CK(cudaGetLastError());
+    }
+    return GP_OK;
+}
+
+static int ensure_scratch(gp_ctx *c, size_t views) {
+    const int cap = c->sc.P;
+    if (c->scratch_views >= views && c->scratch_cap == cap) return GP_OK;
+    CK(cudaDeviceSynchronize());
+    cudaFree(c->d_hdr); cudaFree(c->d_geo); cudaFree(c->d_aux);
+    c->d_hdr = nullptr; c->d_geo = nullptr; c->d_aux = nullptr; c->scratch_views = 0;
+    if (cudaMalloc(&c->d_hdr, views * sizeof(ViewHdr)) != cudaSuccess ||
+        cudaMalloc(&c->d_geo, views * cap * sizeof(EntryGeo)) != cudaSuccess ||
+        cudaMalloc(&c->d_aux, views * cap * sizeof(EntryAux)) != cudaSuccess) {
+        cudaGetLastError();
+        cudaFree(c->d_hdr); cudaFree(c->d_geo); cudaFree(c->d_aux);
+        c->d_hdr = nullptr; c->d_geo = nullptr; c->d_aux = nullptr;
+        return GP_ERR_NOMEM;
+    }
+    c->scratch_views = views; c->scratch_cap = cap;
+    return GP_OK;
+}
+
+static int check_render_args(gp_ctx *c, int world_begin, int n_worlds, int agents, int H, int W, float fov) {
+    if (!c) return GP_ERR_ARG;
+    if (!c->have_scene) return GP_ERR_STATE;
+    if (H < 1 || W < 1 || H > 4096 || W > 4096 || n_worlds < 1 || world_begin < 0) return GP_ERR_ARG;
+    if (!(fov > 0.0f && fov < 3.1415f)) return GP_ERR_ARG;
+    if (agents != c->sc.A || (long long)world_begin + n_worlds > c->sc.Wn) return GP_ERR_RANGE;
+    return GP_OK;
+}
+
+// Enqueue cull + render (or the brute-force kernel) for a world range into DEVICE planes.
+static int render_device(gp_ctx *c, int world_begin, int n_worlds, int H, int W, float fov_rad,
+                         uint8_t *d_class, int32_t *d_instance, float *d_depth, uint8_t *d_rgb,
+                         cudaStream_t stream) {
+    const SceneConst &sc = c->sc;
+    const float th = (float)tan(0.5 * (double)fov_rad);          // C2, host side
+    const float tv = th * ((float)H / (float)W);
+    const size_t views = (size_t)n_worlds * sc.A;
+    if (views > 0x7fffffffull) return GP_ERR_ARG;
+    unsigned long long *stats = c->opt_stats ? c->d_stats : nullptr;
+    if (stats) CK(cudaMemsetAsync(stats, 0, 2 * sizeof(unsigned long long), stream));
+
+    if (c->opt_path == GP_PATH_BRUTE || (W & 3)) {
+        const int HW = H * W;
+        dim3 grid((unsigned)views, (unsigned)std::min((HW + 255) / 256, 65535));
+        {
+            LaunchTimer lt(c, GP_KERNEL_BRUTE, stream);
+            k_render_brute<<<grid, 256, 0, stream>>>(sc, c->d_prims, c->d_pitch, world_begin, H, W, th, tv,
+                                                      d_class, d_instance, d_depth, d_rgb);
+        }
+        c->launches += 1;
+        CK(cudaGetLastError());
+        return GP_OK;
+    }
+    int rc = ensure_scratch(c, views);
+    if (rc != GP_OK) return rc;
+    {
+        LaunchTimer lt(c, GP_KERNEL_CULL, stream);
+        k_cull<<<(unsigned)views, 128, 0, stream>>>(sc, c->d_prims, c->d_pitch, world_begin, H, W, th, tv,
+                                                    c->d_hdr, c->d_geo, c->d_aux, c->scratch_cap, stats);
+    }
+    c->launches += 1;
+    CK(cudaGetLastError());
+
+    RenderArgs ra;
+    ra.hdr = c->d_hdr; ra.geo = c->d_geo; ra.aux = c->d_aux; ra.meta = c->d_meta;
+    ra.cap = c->scratch_cap; ra.world_begin = world_begin; ra.H = H; ra.W = W; ra.th = th; ra.tv = tv;
+    int SR = 1;                                                    // rows per strip: ~512 pixels, power of two
+    while (SR < 16 && SR * 2 * W <= 512) SR *= 2;
+    ra.SR = SR;
+    const int LR = SR < 4 ? SR : 4;
+    ra.log2LC = LR == 4 ? 3 : LR == 2 ? 4 : 5;
+    ra.o_cls = d_class; ra.o_inst = d_instance; ra.o_depth = d_depth; ra.o_rgb = d_rgb; ra.stats = stats;
+    const int n_strips = (H + SR - 1) / SR;
+    const int nwarps = n_strips < 8 ? n_strips : 8;
+    const size_t smem = 16 + (size_t)ra.cap * 64 + (size_t)H * 16 + (size_t)((W + 3) & ~3) * 4 +
+                        (size_t)nwarps * SR * W * 8;
+    if (smem > 227 * 1024) return GP_ERR_ARG;
+    if (smem > c->render_smem_set) {
+        CK(cudaFuncSetAttribute(k_render<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        CK(cudaFuncSetAttribute(k_render<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        c->render_smem_set = smem;
+    }
+    {
+        LaunchTimer lt(c, GP_KERNEL_RENDER, stream);
+        if (stats) k_render<true><<<(unsigned)views, nwarps * 32, smem, stream>>>(sc, ra);
+        else k_render<false><<<(unsigned)views, nwarps * 32, smem, stream>>>(sc, ra);
+    }
+    c->launches += 1;
+    CK(cudaGetLastError());
+    return GP_OK;
+}
+
+extern "C" int gp_render_batch(gp_ctx *c, int world_begin, int n_worlds, int agents, int H, int W,
+                               float fov_rad, uint8_t *d_class, int32_t *d_instance, float *d_depth,
+                               uint8_t *d_rgb, void *stream_) {
+    int rc = check_render_args(c, world_begin, n_worlds, agents, H, W, fov_rad);
+    if (rc != GP_OK) return rc;
+    if (!d_class || !d_instance || !d_depth) return GP_ERR_ARG;
+    if (!aligned16(d_class) || !aligned16(d_instance) || !aligned16(d_depth) || !aligned16(d_rgb)) return GP_ERR_ALIGN;
+    return render_device(c, world_begin, n_worlds, H, W, fov_rad, d_class, d_instance, d_depth, d_rgb,
+                         static_cast<cudaStream_t>(stream_));
+}
+
+extern "C" int gp_render_batch_host(gp_ctx *c, const float *h_pose, int world_begin, int n_worlds, int agents,
+                                    int H, int W, float fov_rad, uint8_t *h_class, int32_t *h_instance,
+                                    float *h_depth, uint8_t *h_rgb, void *stream_) {
+    int rc = check_render_args(c, world_begin, n_worlds, agents, H, W, fov_rad);
+    if (rc != GP_OK) return rc;
+    if (!h_class || !h_instance || !h_depth) return GP_ERR_ARG;
+    cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+    const SceneConst &sc = c->sc;
+    const size_t HW = (size_t)H * W, A = sc.A;
+    const size_t bpv = HW * (h_rgb ? 12 : 9);                     // output bytes per view
+    // chunk: <= 512 MiB of planes per staging buffer, at least one world
+    size_t wc = (512ull << 20) / (bpv * A);
+    if (wc < 1) wc = 1;
+    if (wc > (size_t)n_worlds) wc = n_worlds;
+    const size_t plane = (wc * A * HW + 255) & ~(size_t)255;       // staging plane stride in elements
+    const size_t need = plane * 12;
+    if (!c->copy_stream) {
+        CK(cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
+        for (int i = 0; i < 2; ++i) {
+            CK(cudaEventCreateWithFlags(&c->ev_render[i], cudaEventDisableTiming));
+            CK(cudaEventCreateWithFlags(&c->ev_copy[i], cudaEventDisableTiming));
+        }
+    }
+    if (c->d_out_bytes < need) {
+        CK(cudaDeviceSynchronize());
+        for (int i = 0; i < 2; ++i) { cudaFree(c->d_out[i]); c->d_out[i] = nullptr; }
+        c->d_out_bytes = 0;
+        for (int i = 0; i < 2; ++i)
+            if (cudaMalloc(&c->d_out[i], need) != cudaSuccess) { cudaGetLastError(); return GP_ERR_NOMEM; }
+        c->d_out_bytes = need;
+    }
+    if (h_pose) {
+        CK(cudaMemcpyAsync(c->d_pose, h_pose, (size_t)sc.Wn * A * 4 * sizeof(float), cudaMemcpyHostToDevice, stream));
+        rc = gp_agents_update(c, c->d_pose, stream);
+        if (rc != GP_OK) return rc;
+    }
+    int buf = 0;
+    for (size_t w0 = 0; w0 < (size_t)n_worlds; w0 += wc, buf ^= 1) {
+        const size_t nw = std::min(wc, (size_t)n_worlds - w0), nv = nw * A;
+        unsigned char *base = c->d_out[buf];
+        uint8_t *dc = base; int32_t *di = reinterpret_cast<int32_t *>(base + plane);
+        float *dd = reinterpret_cast<float *>(base + plane * 5);
+        uint8_t *dr = h_rgb ? base + plane * 9 : nullptr;
+        CK(cudaStreamWaitEvent(stream, c->ev_copy[buf], 0));      // staging buffer free again
+        rc = render_device(c, world_begin + (int)w0, (int)nw, H, W, fov_rad, dc, di, dd, dr, stream);
+        if (rc != GP_OK) return rc;
+        CK(cudaEventRecord(c->ev_render[buf], stream));
+        CK(cudaStreamWaitEvent(c->copy_stream, c->ev_render[buf], 0));
+        const size_t v0 = w0 * A;
+        CK(cudaMemcpyAsync(h_class + v0 * HW, dc, nv * HW, cudaMemcpyDeviceToHost, c->copy_stream));
+        CK(cudaMemcpyAsync(h_instance + v0 * HW, di, nv * HW * 4, cudaMemcpyDeviceToHost, c->copy_stream));
+        CK(cudaMemcpyAsync(h_depth + v0 * HW, dd, nv * HW * 4, cudaMemcpyDeviceToHost, c->copy_stream));
+        if (h_rgb) CK(cudaMemcpyAsync(h_rgb + v0 * HW * 3, dr, nv * HW * 3, cudaMemcpyDeviceToHost, c->copy_stream));
+        CK(cudaEventRecord(c->ev_copy[buf], c->copy_stream));
+    }
+    CK(cudaStreamSynchronize(c->copy_stream));
+    CK(cudaStreamSynchronize(stream));
+    return GP_OK;
+}
+
+extern "C" int gp_stats(gp_ctx *c, uint64_t *executed_tests, uint64_t *listed_pairs) {
+    if (!c) return GP_ERR_ARG;
+    unsigned long long h[2];
+    CK(cudaDeviceSynchronize());
+    CK(cudaMemcpy(h, c->d_stats, sizeof h, cudaMemcpyDeviceToHost));
+    if (executed_tests) *executed_tests = h[0];
+    if (listed_pairs) *listed_pairs = h[1];
+    return GP_OK;
+}
+
+extern "C" int gp_kernel_time(gp_ctx *c, int kernel, double *total_ms, uint64_t *launches) {
+    if (!c || !total_ms || !launches) return GP_ERR_ARG;
+    CK(cudaDeviceSynchronize());
+    double ms = 0.0; uint64_t n = 0;
+    std::vector<gp_ctx::Timed> keep;
+    for (const auto &t : c->timed) {
+        if (t.kernel != kernel) { keep.push_back(t); continue; }
+        float x = 0.0f;
+        if (cudaEventElapsedTime(&x, t.a, t.b) == cudaSuccess) { ms += x; ++n; }
+        c->ev_pool.push_back(t.a); c->ev_pool.push_back(t.b);
+    }
+    c->timed.swap(keep);
+    *total_ms = ms; *launches = n;
+    return GP_OK;
+}
+
+extern "C" int gp_launch_count(gp_ctx *c, uint64_t *launches) {
+    if (!c || !launches) return GP_ERR_ARG;
+    *launches = c->launches;
+    return GP_OK;
+}

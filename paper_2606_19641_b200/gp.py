@@ -1,0 +1,176 @@
+"""Thin ctypes binding of libgp.so (include/gp.h).  Argument marshalling only.
+
+torch is used for device memory and the current stream; nothing here computes.  If libgp.so is
+missing (not built) importing the library raises: there is no fallback path.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libgp.so")
+
+GP_OK, GP_ERR_ARG, GP_ERR_ALIGN, GP_ERR_STATE, GP_ERR_RANGE, GP_ERR_CUDA, GP_ERR_ARCH, GP_ERR_NOMEM = \
+    0, -1, -2, -3, -4, -5, -6, -7
+GP_OPT_PATH, GP_OPT_STATS, GP_OPT_TIMING = 1, 2, 3
+GP_KERNEL_UPDATE, GP_KERNEL_CULL, GP_KERNEL_RENDER, GP_KERNEL_BRUTE = 0, 1, 2, 3
+GP_PATH_FAST, GP_PATH_BRUTE = 0, 1
+
+EXPORTS = ("gp_create", "gp_destroy", "gp_set_option", "gp_scene_upload", "gp_agents_update",
+           "gp_cameras_set", "gp_render_batch", "gp_render_batch_host", "gp_stats", "gp_kernel_time",
+           "gp_launch_count",
+           "gp_error_string")
+
+
+class SceneDesc(ctypes.Structure):
+    _fields_ = [("n_worlds", ctypes.c_int32), ("agents_per_world", ctypes.c_int32),
+                ("quads_per_world", ctypes.c_int32), ("cam_height", ctypes.c_float),
+                ("t_max", ctypes.c_float), ("light", ctypes.c_float * 3), ("ambient", ctypes.c_float),
+                ("palette", (ctypes.c_uint8 * 3) * 4)]
+
+
+class GpError(RuntimeError):
+    def __init__(self, code, text):
+        super().__init__("gp error %d: %s" % (code, text))
+        self.code = code
+
+
+_lib = None
+
+
+def lib():
+    """Load libgp.so (raises OSError if it has not been built; see paper_2606_19641_b200/build.py)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise OSError("libgp.so is not built (run `python -m paper_2606_19641_b200.build`); "
+                          "there is no fallback renderer")
+        L = ctypes.CDLL(LIB_PATH)
+        vp, ci, cf = ctypes.c_void_p, ctypes.c_int, ctypes.c_float
+        L.gp_create.argtypes = [ctypes.POINTER(vp), ci]
+        L.gp_destroy.argtypes = [vp]
+        L.gp_set_option.argtypes = [vp, ci, ci]
+        L.gp_scene_upload.argtypes = [vp, ctypes.POINTER(SceneDesc), vp, vp, vp]
+        L.gp_agents_update.argtypes = [vp, vp, vp]
+        L.gp_cameras_set.argtypes = [vp, vp, vp]
+        L.gp_render_batch.argtypes = [vp, ci, ci, ci, ci, ci, cf, vp, vp, vp, vp, vp]
+        L.gp_render_batch_host.argtypes = [vp, vp, ci, ci, ci, ci, ci, cf, vp, vp, vp, vp, vp]
+        L.gp_stats.argtypes = [vp, ctypes.POINTER(ctypes.c_uint64), ctypes.POINTER(ctypes.c_uint64)]
+        L.gp_kernel_time.argtypes = [vp, ci, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_uint64)]
+        L.gp_launch_count.argtypes = [vp, ctypes.POINTER(ctypes.c_uint64)]
+        L.gp_error_string.argtypes = [ci]
+        L.gp_error_string.restype = ctypes.c_char_p
+        for name in EXPORTS[:-1]:
+            getattr(L, name).restype = ci
+        _lib = L
+    return _lib
+
+
+def _check(rc):
+    if rc != GP_OK:
+        raise GpError(rc, lib().gp_error_string(rc).decode())
+
+
+def _stream():
+    import torch
+    return ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def _dptr(t):
+    return None if t is None else ctypes.c_void_p(t.data_ptr())
+
+
+class Renderer:
+    """One gp_ctx.  Methods mirror the C ABI one to one."""
+
+    def __init__(self, device: int = 0):
+        self._h = ctypes.c_void_p()
+        _check(lib().gp_create(ctypes.byref(self._h), int(device)))
+        self.device = int(device)
+        self.desc = None
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib().gp_destroy(self._h)
+            self._h = None
+
+    __del__ = close
+
+    def set_option(self, key: int, value: int):
+        _check(lib().gp_set_option(self._h, key, value))
+
+    def scene_upload(self, agents: np.ndarray, quads: np.ndarray | None, cam_height=1.6, t_max=100.0,
+                     light=(0.48, 0.36, 0.8), ambient=0.25,
+                     palette=((135, 206, 235), (90, 90, 90), (240, 240, 240), (40, 80, 220))):
+        """agents [Wn][A], quads [Wn][Q] (or None): host arrays of 48-byte gp_prim records."""
+        agents = np.ascontiguousarray(agents)
+        assert agents.ndim == 2 and agents.dtype.itemsize == 48
+        Wn, A = agents.shape
+        Q = 0
+        if quads is not None and quads.size:
+            quads = np.ascontiguousarray(quads)
+            assert quads.ndim == 2 and quads.shape[0] == Wn and quads.dtype.itemsize == 48
+            Q = quads.shape[1]
+        d = SceneDesc()
+        d.n_worlds, d.agents_per_world, d.quads_per_world = Wn, A, Q
+        d.cam_height, d.t_max, d.ambient = cam_height, t_max, ambient
+        for i in range(3):
+            d.light[i] = light[i]
+        for c in range(4):
+            for ch in range(3):
+                d.palette[c][ch] = int(palette[c][ch])
+        _check(lib().gp_scene_upload(self._h, ctypes.byref(d), agents.ctypes.data,
+                                     quads.ctypes.data if Q else None, _stream()))
+        self.desc = d
+
+    def agents_update(self, d_pose):
+        """d_pose: CUDA float32 tensor [Wn][A][4] = (cx, cy, cos yaw, sin yaw)."""
+        _check(lib().gp_agents_update(self._h, _dptr(d_pose), _stream()))
+
+    def cameras_set(self, d_pitch_cs=None):
+        """d_pitch_cs: CUDA float32 tensor [Wn][A][2] = (cos p, sin p), or None for pitch 0."""
+        _check(lib().gp_cameras_set(self._h, _dptr(d_pitch_cs), _stream()))
+
+    def render_batch(self, world_begin, n_worlds, H, W, fov_rad, d_class, d_instance, d_depth, d_rgb=None):
+        """Outputs: CUDA tensors uint8 [n][H][W], int32 [n][H][W], float32 [n][H][W], uint8 [n][3][H][W]."""
+        _check(lib().gp_render_batch(self._h, int(world_begin), int(n_worlds), int(self.desc.agents_per_world),
+                                     int(H), int(W), float(fov_rad), _dptr(d_class), _dptr(d_instance),
+                                     _dptr(d_depth), _dptr(d_rgb), _stream()))
+
+    def render_batch_host(self, h_pose, world_begin, n_worlds, H, W, fov_rad, h_class, h_instance, h_depth,
+                          h_rgb=None):
+        """Host-buffer variant (torch CPU tensors, ideally pinned, or numpy arrays)."""
+        def hp(x):
+            if x is None:
+                return None
+            return ctypes.c_void_p(x.ctypes.data if isinstance(x, np.ndarray) else x.data_ptr())
+        _check(lib().gp_render_batch_host(self._h, hp(h_pose), int(world_begin), int(n_worlds),
+                                          int(self.desc.agents_per_world), int(H), int(W), float(fov_rad),
+                                          hp(h_class), hp(h_instance), hp(h_depth), hp(h_rgb), _stream()))
+
+    def stats(self):
+        a, b = ctypes.c_uint64(), ctypes.c_uint64()
+        _check(lib().gp_stats(self._h, ctypes.byref(a), ctypes.byref(b)))
+        return {"executed_tests": a.value, "listed_pairs": b.value}
+
+    def kernel_time(self, kernel: int):
+        """(total_ms, launches) of one kernel since the last call (needs GP_OPT_TIMING = 1)."""
+        ms, n = ctypes.c_double(), ctypes.c_uint64()
+        _check(lib().gp_kernel_time(self._h, kernel, ctypes.byref(ms), ctypes.byref(n)))
+        return ms.value, n.value
+
+    def launch_count(self) -> int:
+        a = ctypes.c_uint64()
+        _check(lib().gp_launch_count(self._h, ctypes.byref(a)))
+        return a.value
+
+    def alloc_outputs(self, n_views, H, W, rgb=True):
+        import torch
+        dev = torch.device("cuda", self.device)
+        return (torch.empty((n_views, H, W), dtype=torch.uint8, device=dev),
+                torch.empty((n_views, H, W), dtype=torch.int32, device=dev),
+                torch.empty((n_views, H, W), dtype=torch.float32, device=dev),
+                torch.empty((n_views, 3, H, W), dtype=torch.uint8, device=dev) if rgb else None)
