@@ -1,0 +1,341 @@
+#!/usr/bin/env python
+"""bench.py — throughput of the render hot path on the paper-scale workload (BASELINE.json configs[2]).
+
+One step = one pass of the whole path over one frame of synthetic input: pose update (a0) ->
+camera setup + frustum cull + compaction (a1, a2) -> render (a3-a9) of 1024 worlds x 64 agents at
+128x128, all four planes.  Poses of consecutive frames (speed / yaw-rate dynamics at dt = 0.1 s) are
+resident in HBM before the timed region.  Prints ONE JSON line (see the driver's contract).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--workload paper|small|...]
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import gp_scenes as gs  # noqa: E402
+
+METRIC = "agent-views rendered/sec at 128x128 (1024 worlds x 64 agents, class+instance+depth+RGB)"
+UNIT = "agent-views/s"
+FP32_OPS_PER_TEST = 29          # contract C5 per executed slab test
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--workload", default="paper", choices=list(gs.CONFIGS))
+    ap.add_argument("--worlds", type=int, default=0, help="override the number of worlds (debug)")
+    ap.add_argument("--res", type=int, default=0, help="override H = W (resolution sweep)")
+    ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    return ap.parse_args()
+
+
+def peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, copy read+write)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            if len(r) < 7:
+                continue
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+            except ValueError:
+                continue
+            for n, v in zip(names, r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def workload_cfg(args):
+    cfg = gs.config(args.workload)
+    if args.worlds:
+        cfg = cfg.replace(n_worlds=args.worlds)
+    if args.res:
+        cfg = cfg.replace(H=args.res, W=args.res)
+    return cfg
+
+
+def config_dict(cfg, extra=None):
+    d = {"workload": "%s: %d worlds x %d agents + %d quads, %dx%d px, %.0f m extent, 4 planes" % (
+        cfg.name, cfg.n_worlds, cfg.agents, cfg.quads, cfg.H, cfg.W, cfg.extent),
+        "baseline_config": "BASELINE.json configs[2] (paper-scale)" if cfg.name == "paper" else cfg.name,
+        "views_per_step": cfg.views, "pixels_per_step": cfg.views * cfg.H * cfg.W,
+        "l2": "outputs per step (%.2f GB) far exceed the 126 MB L2; no explicit flush" % (cfg.views * cfg.H * cfg.W * 12 / 1e9)}
+    if extra:
+        d.update(extra)
+    return d
+
+
+# ------------------------------------------------------------------------------------------------
+def oracle_sample(cfg, n_views, threads):
+    """The oracle as it stands over the first n_views views of the workload (frame 0); returns seconds."""
+    import oracle
+    n_w = (n_views + cfg.agents - 1) // cfg.agents
+    sub = cfg.replace(n_worlds=n_w)
+    agents, quads = gs.gen_world_prims(sub)
+    prims = np.concatenate([agents, quads], axis=1)
+    pitch = gs.gen_pitch(sub) if cfg.pitch_deg_max > 0 else None
+    par = oracle.make_params(cam_height=cfg.cam_height, t_max=cfg.t_max, fov_rad=float(np.float32(cfg.fov_rad)))
+    views = [(v // cfg.agents, v % cfg.agents) for v in range(n_views)]
+    oracle.render_views(prims, views[:threads], cfg.H, cfg.W, par, pitch_cs=pitch, threads=threads)   # page in
+    t0 = time.perf_counter()
+    oracle.render_views(prims, views, cfg.H, cfg.W, par, pitch_cs=pitch, threads=threads)
+    return time.perf_counter() - t0
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle timed on the host cores (rank 0 only)."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    cfg = workload_cfg(args)
+    threads = max(1, min(64, os.cpu_count() or 1))
+    per_core_s = 0.09 * (cfg.H * cfg.W * cfg.prims) / (128 * 128 * 264)
+    n_views = max(threads, int(min(cfg.views, max(1, round(6.0 * threads / per_core_s)))))   # ~6 s per step
+    for _ in range(args.warmup):
+        oracle_sample(cfg, min(n_views, threads), threads)
+    t = [oracle_sample(cfg, n_views, threads) for _ in range(args.steps)]
+    total = sum(t)
+    value = n_views * args.steps / total
+    sample = "%d views of the workload (frame 0) per step, all-primitive fp32 oracle, %d threads" % (n_views, threads)
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": config_dict(cfg, {"sample": sample}),
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+# ------------------------------------------------------------------------------------------------
+def run_b200(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2606_19641_b200 import Renderer, gp
+
+    rank = int(os.environ.get("RANK", "0"))
+    world_size = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    distributed = world_size > 1
+    torch.cuda.set_device(local_rank)
+    if distributed:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    dev = torch.device("cuda", local_rank)
+
+    cfg = workload_cfg(args)
+    # weak scaling: every rank renders its own cfg.n_worlds worlds (rank-disjoint world ids), no collective
+    # on the data path (the path has no exchange step: PAPER.md:319).
+    w0 = rank * cfg.n_worlds
+    agents, quads = gs.gen_world_prims(cfg.replace(n_worlds=w0 + cfg.n_worlds), w0, cfg.n_worlds)
+    big = cfg.replace(n_worlds=w0 + cfg.n_worlds)
+    speed, yaw_rate = gs.gen_dynamics(big, w0, cfg.n_worlds)
+    n_frames = args.steps + args.warmup
+    poses = gs.poses_at_frames(cfg, agents, speed, yaw_rate, range(n_frames))
+    d_pose = torch.from_numpy(np.stack([poses[f] for f in range(n_frames)])).to(dev)   # resident in HBM
+    fov = float(np.float32(cfg.fov_rad))
+
+    r = Renderer(local_rank)
+    r.scene_upload(agents, quads, cam_height=cfg.cam_height, t_max=cfg.t_max)
+    if cfg.pitch_deg_max > 0:
+        r.cameras_set(torch.from_numpy(gs.gen_pitch(big, w0, cfg.n_worlds)).to(dev))
+    outs = r.alloc_outputs(cfg.views, cfg.H, cfg.W, rgb=True)
+
+    def step(f):
+        r.agents_update(d_pose[f])
+        r.render_batch(0, cfg.n_worlds, cfg.H, cfg.W, fov, *outs)
+
+    def barrier():
+        if distributed:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for f in range(args.warmup):
+        step(f)
+    barrier()
+    r.set_option(gp.GP_OPT_TIMING, 1)
+    for k in (gp.GP_KERNEL_UPDATE, gp.GP_KERNEL_CULL, gp.GP_KERNEL_RENDER):
+        r.kernel_time(k)
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+    launches0 = r.launch_count()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    ev0.record()
+    for f in range(args.warmup, n_frames):
+        step(f)
+    ev1.record()
+    barrier()
+    ms = ev0.elapsed_time(ev1)
+    clocks = sampler.stop() if rank == 0 else None
+    launches = r.launch_count() - launches0
+    ktimes = {name: r.kernel_time(k) for name, k in (("update", gp.GP_KERNEL_UPDATE), ("cull", gp.GP_KERNEL_CULL),
+                                                       ("render", gp.GP_KERNEL_RENDER))}
+    r.set_option(gp.GP_OPT_TIMING, 0)
+    if distributed:
+        t = torch.tensor([ms], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+
+    # one instrumented frame (not timed): executed tests and listed pairs for the FP32 roof
+    r.set_option(gp.GP_OPT_STATS, 1)
+    step(n_frames - 1)
+    stats = r.stats()
+    r.set_option(gp.GP_OPT_STATS, 0)
+
+    # end to end through the host-buffer entry point (pinned host memory, copies inside the timed region)
+    e2e = None
+    if not args.no_e2e:
+        try:
+            V, H, W = cfg.views, cfg.H, cfg.W
+            h = [torch.empty((V, H, W), dtype=torch.uint8), torch.empty((V, H, W), dtype=torch.int32),
+                 torch.empty((V, H, W), dtype=torch.float32), torch.empty((V, 3, H, W), dtype=torch.uint8)]
+            pinned = True
+            try:
+                h = [x.pin_memory() for x in h]
+            except RuntimeError:
+                pinned = False
+            h_pose = [torch.from_numpy(poses[f]).pin_memory() if pinned else torch.from_numpy(poses[f])
+                      for f in range(min(n_frames, args.e2e_steps + 1))]
+            r.render_batch_host(h_pose[0], 0, cfg.n_worlds, H, W, fov, *h)            # warm-up, allocates staging
+            barrier()
+            t0 = time.perf_counter()
+            for i in range(args.e2e_steps):
+                r.render_batch_host(h_pose[(i + 1) % len(h_pose)], 0, cfg.n_worlds, H, W, fov, *h)   # synchronises
+            barrier()
+            e_s = time.perf_counter() - t0
+            if distributed:
+                t = torch.tensor([e_s], device=dev, dtype=torch.float64)
+                dist.all_reduce(t, op=dist.ReduceOp.MAX)
+                e_s = float(t.item())
+            e2e = {"value": world_size * cfg.views * args.e2e_steps / e_s, "unit": UNIT,
+                   "h2d_bytes_per_step": int(h_pose[0].numel() * 4),
+                   "d2h_bytes_per_step": int(sum(x.numel() * x.element_size() for x in h)),
+                   "steps": args.e2e_steps, "pinned_host": pinned,
+                   "api": "gp_render_batch_host (H2D poses, render in chunks, D2H of all four planes)"}
+            del h
+        except Exception as ex:  # noqa: BLE001 - report, do not hide
+            e2e = {"value": None, "unit": UNIT, "error": repr(ex)[:200]}
+
+    if rank != 0:
+        if distributed:
+            dist.destroy_process_group()
+        return
+
+    views_total = world_size * cfg.views * args.steps
+    value = views_total / (ms * 1e-3)
+    npx = cfg.views * cfg.H * cfg.W
+    peak, peak_src = peaks()
+    alg_bytes = npx * 12 + cfg.n_worlds * cfg.prims * 48 + cfg.views * 64
+    r_ms, r_n = ktimes["render"]
+    r_avg_ms = r_ms / max(1, r_n)
+    achieved = alg_bytes / (r_avg_ms * 1e-3) / 1e9
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tpath):
+        with open(tpath) as f:
+            traffic = json.load(f).get(cfg.name)
+    sm_mhz = (clocks or {}).get("sm_mhz") or 1965.0
+    fp32_peak = 148 * 128 * 2 * sm_mhz * 1e6
+    t_fp32_ms = stats["executed_tests"] * FP32_OPS_PER_TEST / fp32_peak * 1e3
+    t_hbm_ms = alg_bytes / (peak * 1e9) * 1e3
+    step_ms = ms / args.steps
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world_size, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": step_ms, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": config_dict(cfg),
+        "mpixels_per_s": value * cfg.H * cfg.W / 1e6,
+        "clocks": clocks,
+        "gpu_launches": int(launches),
+        "kernels_ms_per_step": {k: v[0] / max(1, v[1]) for k, v in ktimes.items()},
+        "roofline": {"bound": "hbm", "kernel": "k_render", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                     "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
+                     "algorithmic_bytes_per_launch": alg_bytes, "avg_launch_ms": r_avg_ms,
+                     "share_of_step": r_avg_ms / step_ms},
+        "roofline_step": {"t_hbm_ms": t_hbm_ms, "t_fp32_ms": t_fp32_ms, "frac_of_slower_roof": max(t_hbm_ms, t_fp32_ms) / step_ms,
+                          "executed_tests": stats["executed_tests"], "listed_pairs": stats["listed_pairs"],
+                          "tests_per_pixel": stats["executed_tests"] / npx, "fp32_peak_tflops": fp32_peak / 1e12,
+                          "fp32_ops_per_test": FP32_OPS_PER_TEST},
+        "e2e": e2e,
+    }
+    if not args.no_cpu_baseline and world_size == 1:
+        threads = max(1, min(64, os.cpu_count() or 1))
+        per_core_s = 0.09 * (cfg.H * cfg.W * cfg.prims) / (128 * 128 * 264)
+        n_views = int(min(cfg.views, max(threads, round(12.0 * threads / per_core_s))))
+        sec = oracle_sample(cfg, n_views, threads)
+        out["cpu_baseline"] = {"value": n_views / sec, "unit": UNIT, "cores": threads, "kind": "oracle",
+                               "sample": "%d views of the workload (frame 0), all-primitive fp32 oracle (oracle/gp_oracle.c), %d threads, %.1f s"
+                                         % (n_views, threads, sec)}
+    print(json.dumps(out))
+    if distributed:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_b200(args)
+
+
+if __name__ == "__main__":
+    main()

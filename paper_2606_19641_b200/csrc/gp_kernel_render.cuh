@@ -92,13 +92,21 @@ k_render(SceneConst sc, RenderArgs ra) {
     if (n > 0) mbar_wait(bar, 0);
 
     const int w = ra.world_begin + view / sc.A;
-    const PrimMeta *wmeta = ra.meta + (size_t)w * sc.P;
+    const uint32_t *wtab = reinterpret_cast<const uint32_t *>(ra.meta + (size_t)w * sc.P);   // uint32[P][8]
     const int s8_ground = shade_scale(c_max(sc.Lz, 0.0f), sc.ambient);
     const uint32_t rgb_ground = shade_rgb(sc.pal[1], s8_ground), rgb_sky = sc.pal[0];
+    const uint32_t gr4 = (rgb_ground & 0xff) * 0x01010101u, gg4 = ((rgb_ground >> 8) & 0xff) * 0x01010101u,
+                   gb4 = ((rgb_ground >> 16) & 0xff) * 0x01010101u;
+    const uint32_t sr4 = (rgb_sky & 0xff) * 0x01010101u, sg4 = ((rgb_sky >> 8) & 0xff) * 0x01010101u,
+                   sb4 = ((rgb_sky >> 16) & 0xff) * 0x01010101u;
     const int LC = 1 << ra.log2LC, LR = 32 >> ra.log2LC;
     const int li = lane >> ra.log2LC, lj = lane & (LC - 1);
     const size_t HW = (size_t)H * W;
     const int n_strips = (H + SR - 1) / SR;
+    // resolve pass: lane owns pixels 4*lane .. 4*lane+3 of every 128-pixel group of the strip
+    const int lane_row = (lane * 4) / W, lane_col = (lane * 4) % W;
+    const int step_row = 128 / W, step_col = 128 % W;
+    const float t_max = sc.t_max;
     unsigned long long n_tests = 0;
 
     for (int strip = warp; strip < n_strips; strip += nwarps) {
@@ -123,14 +131,19 @@ k_render(SceneConst sc, RenderArgs ra) {
             while (mask) {
                 const int eb = base + __ffs(mask) - 1;
                 mask &= mask - 1;
-                const float4 g0 = *reinterpret_cast<const float4 *>(&s_geo[eb]);
-                const float4 g1 = *(reinterpret_cast<const float4 *>(&s_geo[eb]) + 1);
-                const float4 g2 = *(reinterpret_cast<const float4 *>(&s_geo[eb]) + 2);
+                const float4 g0 = *reinterpret_cast<const float4 *>(&s_geo[eb]);          // ax bx ay by
+                const float4 g1 = *(reinterpret_cast<const float4 *>(&s_geo[eb]) + 1);    // az bz flx fly
+                const float4 g2 = *(reinterpret_cast<const float4 *>(&s_geo[eb]) + 2);    // rlx rly ulx uly
                 const uint4 ax = *reinterpret_cast<const uint4 *>(&s_aux[eb]);
                 const bool flat = ax.x & 1u;
                 const uint32_t klow = (ax.x >> 1) << 3;
                 const int r0 = max((int)(ax.y & 0xffff), row0), r1 = min((int)(ax.y >> 16), row1);
                 const int c0 = (int)(ax.z & 0xffff), c1 = (int)(ax.z >> 16);
+                // conservative pre-test data (not contract arithmetic): box centre / half extents in
+                // the ray-origin frame, recovered from a = -h - ol, b = h - ol
+                const float mx = 0.5f * (g0.x + g0.y), my = 0.5f * (g0.z + g0.w), mz = 0.5f * (g1.x + g1.y);   // -ol
+                const float ex_ = 0.5f * (g0.y - g0.x), ey_ = 0.5f * (g0.w - g0.z), ez_ = 0.5f * (g1.y - g1.x); // h
+                const float kSlack = 2e-5f, kGrow = 1.00002f;
                 for (int rb = r0; rb <= r1; rb += LR) {
                     const int i = rb + li;
                     for (int cb = c0; cb <= c1; cb += LC) {
@@ -142,26 +155,40 @@ k_render(SceneConst sc, RenderArgs ra) {
                             // C5, per-pixel part
                             const float dlx = c_fma(rt.x, g2.z, c_fma(s, g2.x, g1.z));
                             const float dly = c_fma(rt.x, g2.w, c_fma(s, g2.y, g1.w));
-                            const float ix = c_rcp(dlx), iy = c_rcp(dly);
-                            float ta, tb;
-                            ta = c_mul(g0.x, ix); tb = c_mul(g0.y, ix);
-                            const float lox = c_min(ta, tb), hix = c_max(ta, tb);
-                            ta = c_mul(g0.z, iy); tb = c_mul(g0.w, iy);
-                            const float loy = c_min(ta, tb), hiy = c_max(ta, tb);
-                            ta = c_mul(g1.x, rt.z); tb = c_mul(g1.y, rt.z);
-                            const float loz = c_min(ta, tb), hiz = c_max(ta, tb);
-                            const float tn = c_max(c_max(lox, loy), loz);
-                            const float tf = c_min(c_min(hix, hiy), hiz);
-                            if (tn <= tf && tn > 0.0f && tn <= sc.t_max) {
-                                uint32_t face;                                  // m*2 + (sigma > 0)
-                                if (flat) face = 5;
-                                else if (lox == tn) face = 0 + (dlx > 0.0f ? 0 : 1);
-                                else if (loy == tn) face = 2 + (dly > 0.0f ? 0 : 1);
-                                else face = 4 + (rt.y > 0.0f ? 0 : 1);
-                                const unsigned long long key =
-                                    ((unsigned long long)__float_as_uint(tn) << 32) | klow | face;   // C6
-                                unsigned long long *kp = &keys[(i - row0) * W + j];
-                                if (key < *kp) *kp = key;
+                            const float dlz = rt.y;
+                            // a3 early-out per ray: separating-axis test of the LINE o + t d against the box
+                            // (axes d x e_m).  Division-free; the slack keeps it conservative, so a ray it
+                            // rejects can never pass the exact slab test below.
+                            const float adx = fabsf(dlx), ady = fabsf(dly), adz = fabsf(dlz);
+                            const float px_ = my * dlz, qx_ = mz * dly;
+                            const float py_ = mz * dlx, qy_ = mx * dlz;
+                            const float pz_ = mx * dly, qz_ = my * dlx;
+                            const bool sep =
+                                fabsf(px_ - qx_) > fmaf(ey_, adz, ez_ * ady) * kGrow + kSlack * (fabsf(px_) + fabsf(qx_)) + 1e-12f ||
+                                fabsf(py_ - qy_) > fmaf(ez_, adx, ex_ * adz) * kGrow + kSlack * (fabsf(py_) + fabsf(qy_)) + 1e-12f ||
+                                fabsf(pz_ - qz_) > fmaf(ex_, ady, ey_ * adx) * kGrow + kSlack * (fabsf(pz_) + fabsf(qz_)) + 1e-12f;
+                            if (!sep) {
+                                const float ix = c_rcp(dlx), iy = c_rcp(dly);
+                                float ta, tb;
+                                ta = c_mul(g0.x, ix); tb = c_mul(g0.y, ix);
+                                const float lox = c_min(ta, tb), hix = c_max(ta, tb);
+                                ta = c_mul(g0.z, iy); tb = c_mul(g0.w, iy);
+                                const float loy = c_min(ta, tb), hiy = c_max(ta, tb);
+                                ta = c_mul(g1.x, rt.z); tb = c_mul(g1.y, rt.z);
+                                const float loz = c_min(ta, tb), hiz = c_max(ta, tb);
+                                const float tn = c_max(c_max(lox, loy), loz);
+                                const float tf = c_min(c_min(hix, hiy), hiz);
+                                if (tn <= tf && tn > 0.0f && tn <= t_max) {
+                                    uint32_t face;                                  // m*2 + (sigma > 0)
+                                    if (flat) face = 5;
+                                    else if (lox == tn) face = 0 + (dlx > 0.0f ? 0 : 1);
+                                    else if (loy == tn) face = 2 + (dly > 0.0f ? 0 : 1);
+                                    else face = 4 + (dlz > 0.0f ? 0 : 1);
+                                    const unsigned long long key =
+                                        ((unsigned long long)__float_as_uint(tn) << 32) | klow | face;   // C6
+                                    unsigned long long *kp = &keys[(i - row0) * W + j];
+                                    if (key < *kp) *kp = key;
+                                }
                             }
                         }
                     }
@@ -170,57 +197,57 @@ k_render(SceneConst sc, RenderArgs ra) {
             }
         }
         // ---- a5 ground, a7 resolve, a8 shade, a9 store: 4 consecutive pixels per lane ----------
-        const int nquads = (row1 - row0 + 1) * W / 4;
-        const size_t vbase = (size_t)view * HW + (size_t)row0 * W;
-        for (int q = lane; q < nquads; q += 32) {
-            const int p = q * 4;
-            const int i = row0 + p / W;
-            const float tg = s_row[i].w;
-            const bool ground = tg > 0.0f;
-            uint32_t cls4 = ground ? 0x01010101u : 0u;
-            int4 inst4 = make_int4(-1, -1, -1, -1);
-            const float d0 = ground ? tg : 0.0f;
-            float4 dep4 = make_float4(d0, d0, d0, d0);
-            const uint32_t bg = ground ? rgb_ground : rgb_sky;
-            uint32_t r4 = (bg & 0xff) * 0x01010101u, g4 = ((bg >> 8) & 0xff) * 0x01010101u,
-                     b4 = ((bg >> 16) & 0xff) * 0x01010101u;
-            if (any) {
-                const ulonglong2 ka = *reinterpret_cast<const ulonglong2 *>(&keys[p]);
-                const ulonglong2 kb = *reinterpret_cast<const ulonglong2 *>(&keys[p + 2]);
-                const unsigned long long kk[4] = {ka.x, ka.y, kb.x, kb.y};
-                if ((ka.x & ka.y & kb.x & kb.y) != kKeyEmpty) {
-#pragma unroll
-                    for (int u = 0; u < 4; ++u) {
-                        if (kk[u] == kKeyEmpty) continue;
-                        const float t = __uint_as_float((uint32_t)(kk[u] >> 32));
-                        if (ground && !(t <= tg)) continue;                // the ground is nearer (C6)
-                        const uint32_t lo = (uint32_t)kk[u];
-                        const uint4 m = __ldg(reinterpret_cast<const uint4 *>(&wmeta[lo >> 3]));
-                        const uint32_t face = lo & 7u;
-                        const uint32_t sw = face < 2 ? m.y : face < 4 ? m.z : m.w;
-                        const int s8 = (int)((face & 1u) ? (sw >> 16) : (sw & 0xffffu)) & 0x1ff;
-                        const uint32_t c = (m.y >> 12) & 0xfu;
-                        const uint32_t rgb = c == 0 ? sc.pal[0] : shade_rgb(sc.pal[c & 3], s8);
-                        const int sh = u * 8;
-                        const uint32_t keep = ~(0xffu << sh);
-                        cls4 = (cls4 & keep) | (c << sh);
-                        r4 = (r4 & keep) | ((rgb & 0xff) << sh);
-                        g4 = (g4 & keep) | (((rgb >> 8) & 0xff) << sh);
-                        b4 = (b4 & keep) | (((rgb >> 16) & 0xff) << sh);
-                        (&inst4.x)[u] = (int)m.x;
-                        (&dep4.x)[u] = t;
+        {
+            int row = row0 + lane_row, col = lane_col;
+            uint8_t *pc = ra.o_cls + (size_t)view * HW;
+            int32_t *pi = ra.o_inst + (size_t)view * HW;
+            float *pd = ra.o_depth + (size_t)view * HW;
+            uint8_t *pr = ra.o_rgb ? ra.o_rgb + (size_t)view * 3 * HW : nullptr;
+            while (row <= row1) {
+                const float tg = s_row[row].w;
+                const bool ground = tg > 0.0f;
+                uint32_t cls4 = ground ? 0x01010101u : 0u;
+                int4 inst4 = make_int4(-1, -1, -1, -1);
+                const float d0 = ground ? tg : 0.0f;
+                float4 dep4 = make_float4(d0, d0, d0, d0);
+                uint32_t r4 = ground ? gr4 : sr4, g4 = ground ? gg4 : sg4, b4 = ground ? gb4 : sb4;
+                if (any) {
+                    const unsigned long long *kq = &keys[(row - row0) * W + col];
+                    const ulonglong2 ka = *reinterpret_cast<const ulonglong2 *>(kq);
+                    const ulonglong2 kb = *reinterpret_cast<const ulonglong2 *>(kq + 2);
+                    if ((ka.x & ka.y & kb.x & kb.y) != kKeyEmpty) {
+#define GP_PATCH(KEY, U, SEL, IF, DF)                                                          \
+                        if ((KEY) != kKeyEmpty) {                                              \
+                            const float t = __uint_as_float((uint32_t)((KEY) >> 32));          \
+                            if (!ground || t <= tg) {              /* else the ground is nearer (C6) */ \
+                                const uint32_t lo = (uint32_t)(KEY);                           \
+                                const uint32_t cw = __ldg(&wtab[lo]);                          \
+                                IF = (int)__ldg(&wtab[(lo & ~7u) + 6]);                        \
+                                DF = t;                                                        \
+                                cls4 = __byte_perm(cls4, cw >> 24, SEL);                       \
+                                r4 = __byte_perm(r4, cw, SEL);                                 \
+                                g4 = __byte_perm(g4, cw >> 8, SEL);                            \
+                                b4 = __byte_perm(b4, cw >> 16, SEL);                           \
+                            }                                                                  \
+                        }
+                        GP_PATCH(ka.x, 0, 0x3214, inst4.x, dep4.x)
+                        GP_PATCH(ka.y, 1, 0x3240, inst4.y, dep4.y)
+                        GP_PATCH(kb.x, 2, 0x3410, inst4.z, dep4.z)
+                        GP_PATCH(kb.y, 3, 0x4210, inst4.w, dep4.w)
+#undef GP_PATCH
                     }
                 }
-            }
-            const size_t o = vbase + p;
-            *reinterpret_cast<uint32_t *>(ra.o_cls + o) = cls4;
-            *reinterpret_cast<int4 *>(ra.o_inst + o) = inst4;
-            *reinterpret_cast<float4 *>(ra.o_depth + o) = dep4;
-            if (ra.o_rgb) {
-                uint8_t *rb = ra.o_rgb + (size_t)view * 3 * HW + (size_t)row0 * W + p;
-                *reinterpret_cast<uint32_t *>(rb) = r4;
-                *reinterpret_cast<uint32_t *>(rb + HW) = g4;
-                *reinterpret_cast<uint32_t *>(rb + 2 * HW) = b4;
+                const size_t o = (size_t)row * W + col;
+                *reinterpret_cast<uint32_t *>(pc + o) = cls4;
+                *reinterpret_cast<int4 *>(pi + o) = inst4;
+                *reinterpret_cast<float4 *>(pd + o) = dep4;
+                if (pr) {
+                    *reinterpret_cast<uint32_t *>(pr + o) = r4;
+                    *reinterpret_cast<uint32_t *>(pr + HW + o) = g4;
+                    *reinterpret_cast<uint32_t *>(pr + 2 * HW + o) = b4;
+                }
+                row += step_row; col += step_col;
+                if (col >= W) { col -= W; ++row; }
             }
         }
         __syncwarp();      // the key buffer is reused by this warp's next strip

@@ -11,13 +11,15 @@ __device__ __forceinline__ void write_meta(const gp_prim &p, PrimMeta *out, cons
     float qy = c_fma(p.cos_yaw, sc.Ly, -c_mul(p.sin_yaw, sc.Lx));
     float q[3] = {qx, qy, sc.Lz};
     PrimMeta m;
-    m.inst = p.inst;
+    m.inst = p.inst; m.pad = 0;
+    const uint32_t c = (uint32_t)p.cls & 3u;
 #pragma unroll
     for (int a = 0; a < 3; ++a) {
-        m.s[a * 2 + 0] = (uint16_t)shade_scale(c_max(-q[a], 0.0f), sc.ambient);   // sigma = -1
-        m.s[a * 2 + 1] = (uint16_t)shade_scale(c_max(q[a], 0.0f), sc.ambient);    // sigma = +1
+        const int lo = shade_scale(c_max(-q[a], 0.0f), sc.ambient);    // sigma = -1
+        const int hi = shade_scale(c_max(q[a], 0.0f), sc.ambient);     // sigma = +1
+        m.face[a * 2 + 0] = (c == 0 ? sc.pal[0] : shade_rgb(sc.pal[c], lo)) | (c << 24);
+        m.face[a * 2 + 1] = (c == 0 ? sc.pal[0] : shade_rgb(sc.pal[c], hi)) | (c << 24);
     }
-    m.s[0] = (uint16_t)(m.s[0] | ((p.cls & 0xf) << 12));
     *out = m;
 }
 
