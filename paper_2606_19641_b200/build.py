@@ -21,7 +21,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if not force and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(s) for s in sources()):
         return LIB
     tmp = LIB + ".tmp.%d" % os.getpid()
-    cmd = [NVCC, *FLAGS, *(["-Xptxas", "-v"] if verbose else []), os.path.join(CSRC, "gp_lib.cu"), "-o", tmp]
+    extra = os.environ.get("GP_NVCC_EXTRA", "").split()
+    cmd = [NVCC, *FLAGS, *extra, *(["-Xptxas", "-v"] if verbose else []), os.path.join(CSRC, "gp_lib.cu"), "-o", tmp]
     subprocess.check_call(cmd)
     os.replace(tmp, LIB)
     return LIB

@@ -21,6 +21,7 @@ struct RenderArgs {
     int cap, world_begin, H, W;
     float th, tv;
     int SR, log2LC;                 // rows per strip; lanes per row of the test tile (LC = 1 << log2LC)
+    int log2W;                      // valid when the FAST4 resolve is used (W a power of two)
     uint8_t *o_cls; int32_t *o_inst; float *o_depth; uint8_t *o_rgb;
     unsigned long long *stats;
 };
@@ -46,8 +47,58 @@ __device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t by
 
 constexpr unsigned long long kKeyEmpty = 0xFFFFFFFFFFFFFFFFull;
 
-template <bool STATS>
-__global__ void __launch_bounds__(256)
+// a5/a7/a8/a9 for the 4 consecutive pixels a lane owns in one 128-pixel group: ground / sky default
+// from the row's t_ground, patched where a primitive's key won, then one 4-byte store per 8-bit
+// plane and one 16-byte store per 32-bit plane.
+__device__ __forceinline__ void resolve_quad(float tg, const uint4 *s_bg, const unsigned long long *kq,
+                                             const uint32_t *__restrict__ wtab, uint8_t *pc, int32_t *pi,
+                                             float *pd, uint8_t *pr, size_t HW) {
+    const bool ground = tg > 0.0f;
+    const uint4 bg = s_bg[ground ? 1 : 0];                 // cls4, r4, g4, b4 of the background
+    uint32_t cls4 = bg.x, r4 = bg.y, g4 = bg.z, b4 = bg.w;
+    int4 inst4 = make_int4(-1, -1, -1, -1);
+    const float d0 = fmaxf(tg, 0.0f);                      // tg = -1 marks "no ground on this row"
+    float4 dep4 = make_float4(d0, d0, d0, d0);
+    if (kq) {
+        const ulonglong2 ka = *reinterpret_cast<const ulonglong2 *>(kq);
+        const ulonglong2 kb = *reinterpret_cast<const ulonglong2 *>(kq + 2);
+        if ((ka.x & ka.y & kb.x & kb.y) != kKeyEmpty) {
+#define GP_PATCH(KEY, SEL, IF, DF)                                                             \
+            if ((KEY) != kKeyEmpty) {                                                          \
+                const float t = __uint_as_float((uint32_t)((KEY) >> 32));                      \
+                if (!ground || t <= tg) {                  /* else the ground is nearer (C6) */ \
+                    const uint32_t lo = (uint32_t)(KEY);                                       \
+                    const uint32_t cw = __ldg(&wtab[lo]);                                      \
+                    IF = (int)__ldg(&wtab[lo | 6u]);       /* face codes are 0..5: lo|6 = slot 6 or 7 */ \
+                    DF = t;                                                                    \
+                    cls4 = __byte_perm(cls4, cw >> 24, SEL);                                   \
+                    r4 = __byte_perm(r4, cw, SEL);                                             \
+                    g4 = __byte_perm(g4, cw >> 8, SEL);                                        \
+                    b4 = __byte_perm(b4, cw >> 16, SEL);                                       \
+                }                                                                              \
+            }
+            GP_PATCH(ka.x, 0x3214, inst4.x, dep4.x)
+            GP_PATCH(ka.y, 0x3240, inst4.y, dep4.y)
+            GP_PATCH(kb.x, 0x3410, inst4.z, dep4.z)
+            GP_PATCH(kb.y, 0x4210, inst4.w, dep4.w)
+#undef GP_PATCH
+        }
+    }
+    *reinterpret_cast<uint32_t *>(pc) = cls4;
+    *reinterpret_cast<int4 *>(pi) = inst4;
+    *reinterpret_cast<float4 *>(pd) = dep4;
+    if (pr) {
+        *reinterpret_cast<uint32_t *>(pr) = r4;
+        *reinterpret_cast<uint32_t *>(pr + HW) = g4;
+        *reinterpret_cast<uint32_t *>(pr + 2 * HW) = b4;
+    }
+}
+
+#ifndef GP_RENDER_MIN_CTAS
+#define GP_RENDER_MIN_CTAS 4
+#endif
+template <bool STATS, bool FAST4>
+__global__ void __launch_bounds__(256, GP_RENDER_MIN_CTAS)
 k_render(SceneConst sc, RenderArgs ra) {
     extern __shared__ __align__(16) unsigned char smem[];
     const int view = blockIdx.x;
@@ -56,9 +107,10 @@ k_render(SceneConst sc, RenderArgs ra) {
 
     // ---- shared memory carve-up ---------------------------------------------------------------
     uint64_t *bar = reinterpret_cast<uint64_t *>(smem);
-    EntryGeo *s_geo = reinterpret_cast<EntryGeo *>(smem + 16);
-    EntryAux *s_aux = reinterpret_cast<EntryAux *>(smem + 16 + (size_t)ra.cap * 48);
-    float4 *s_row = reinterpret_cast<float4 *>(smem + 16 + (size_t)ra.cap * 64);
+    uint4 *s_bg = reinterpret_cast<uint4 *>(smem + 16);            // [0] sky, [1] ground: cls4, r4, g4, b4
+    EntryGeo *s_geo = reinterpret_cast<EntryGeo *>(smem + 48);
+    EntryAux *s_aux = reinterpret_cast<EntryAux *>(smem + 48 + (size_t)ra.cap * 48);
+    float4 *s_row = reinterpret_cast<float4 *>(smem + 48 + (size_t)ra.cap * 64);
     float *s_col = reinterpret_cast<float *>(s_row + H);
     unsigned long long *s_keys = reinterpret_cast<unsigned long long *>(s_col + ((W + 3) & ~3));
     unsigned long long *keys = s_keys + (size_t)warp * SR * W;
@@ -66,6 +118,12 @@ k_render(SceneConst sc, RenderArgs ra) {
     const float4 vh4 = __ldg(reinterpret_cast<const float4 *>(&ra.hdr[view]));
     ViewHdr vh; vh.n = __float_as_int(vh4.x); vh.oz = vh4.y; vh.cp = vh4.z; vh.sp = vh4.w;
     const int n = vh.n;
+    if (threadIdx.x == 32 % blockDim.x) {
+        const uint32_t g = shade_rgb(sc.pal[1], shade_scale(c_max(sc.Lz, 0.0f), sc.ambient)), k = sc.pal[0];
+        s_bg[0] = make_uint4(0u, (k & 0xff) * 0x01010101u, ((k >> 8) & 0xff) * 0x01010101u, ((k >> 16) & 0xff) * 0x01010101u);
+        s_bg[1] = make_uint4(0x01010101u, (g & 0xff) * 0x01010101u, ((g >> 8) & 0xff) * 0x01010101u,
+                             ((g >> 16) & 0xff) * 0x01010101u);
+    }
     if (threadIdx.x == 0) {
         mbar_init(bar, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -93,12 +151,6 @@ k_render(SceneConst sc, RenderArgs ra) {
 
     const int w = ra.world_begin + view / sc.A;
     const uint32_t *wtab = reinterpret_cast<const uint32_t *>(ra.meta + (size_t)w * sc.P);   // uint32[P][8]
-    const int s8_ground = shade_scale(c_max(sc.Lz, 0.0f), sc.ambient);
-    const uint32_t rgb_ground = shade_rgb(sc.pal[1], s8_ground), rgb_sky = sc.pal[0];
-    const uint32_t gr4 = (rgb_ground & 0xff) * 0x01010101u, gg4 = ((rgb_ground >> 8) & 0xff) * 0x01010101u,
-                   gb4 = ((rgb_ground >> 16) & 0xff) * 0x01010101u;
-    const uint32_t sr4 = (rgb_sky & 0xff) * 0x01010101u, sg4 = ((rgb_sky >> 8) & 0xff) * 0x01010101u,
-                   sb4 = ((rgb_sky >> 16) & 0xff) * 0x01010101u;
     const int LC = 1 << ra.log2LC, LR = 32 >> ra.log2LC;
     const int li = lane >> ra.log2LC, lj = lane & (LC - 1);
     const size_t HW = (size_t)H * W;
@@ -198,56 +250,27 @@ k_render(SceneConst sc, RenderArgs ra) {
         }
         // ---- a5 ground, a7 resolve, a8 shade, a9 store: 4 consecutive pixels per lane ----------
         {
-            int row = row0 + lane_row, col = lane_col;
-            uint8_t *pc = ra.o_cls + (size_t)view * HW;
-            int32_t *pi = ra.o_inst + (size_t)view * HW;
-            float *pd = ra.o_depth + (size_t)view * HW;
-            uint8_t *pr = ra.o_rgb ? ra.o_rgb + (size_t)view * 3 * HW : nullptr;
-            while (row <= row1) {
-                const float tg = s_row[row].w;
-                const bool ground = tg > 0.0f;
-                uint32_t cls4 = ground ? 0x01010101u : 0u;
-                int4 inst4 = make_int4(-1, -1, -1, -1);
-                const float d0 = ground ? tg : 0.0f;
-                float4 dep4 = make_float4(d0, d0, d0, d0);
-                uint32_t r4 = ground ? gr4 : sr4, g4 = ground ? gg4 : sg4, b4 = ground ? gb4 : sb4;
-                if (any) {
-                    const unsigned long long *kq = &keys[(row - row0) * W + col];
-                    const ulonglong2 ka = *reinterpret_cast<const ulonglong2 *>(kq);
-                    const ulonglong2 kb = *reinterpret_cast<const ulonglong2 *>(kq + 2);
-                    if ((ka.x & ka.y & kb.x & kb.y) != kKeyEmpty) {
-#define GP_PATCH(KEY, U, SEL, IF, DF)                                                          \
-                        if ((KEY) != kKeyEmpty) {                                              \
-                            const float t = __uint_as_float((uint32_t)((KEY) >> 32));          \
-                            if (!ground || t <= tg) {              /* else the ground is nearer (C6) */ \
-                                const uint32_t lo = (uint32_t)(KEY);                           \
-                                const uint32_t cw = __ldg(&wtab[lo]);                          \
-                                IF = (int)__ldg(&wtab[(lo & ~7u) + 6]);                        \
-                                DF = t;                                                        \
-                                cls4 = __byte_perm(cls4, cw >> 24, SEL);                       \
-                                r4 = __byte_perm(r4, cw, SEL);                                 \
-                                g4 = __byte_perm(g4, cw >> 8, SEL);                            \
-                                b4 = __byte_perm(b4, cw >> 16, SEL);                           \
-                            }                                                                  \
-                        }
-                        GP_PATCH(ka.x, 0, 0x3214, inst4.x, dep4.x)
-                        GP_PATCH(ka.y, 1, 0x3240, inst4.y, dep4.y)
-                        GP_PATCH(kb.x, 2, 0x3410, inst4.z, dep4.z)
-                        GP_PATCH(kb.y, 3, 0x4210, inst4.w, dep4.w)
-#undef GP_PATCH
-                    }
+            const size_t o0 = (size_t)view * HW + (size_t)row0 * W + lane * 4;
+            uint8_t *pc = ra.o_cls + o0;
+            int32_t *pi = ra.o_inst + o0;
+            float *pd = ra.o_depth + o0;
+            uint8_t *pr = ra.o_rgb ? ra.o_rgb + 2 * (size_t)view * HW + o0 : nullptr;
+            const unsigned long long *kq = any ? keys + lane * 4 : nullptr;
+            if (FAST4) {        // strip = 512 pixels = 4 groups, W a power of two: constant offsets
+#pragma unroll
+                for (int it = 0; it < 4; ++it) {
+                    const int row = row0 + ((lane * 4 + it * 128) >> ra.log2W);
+                    resolve_quad(s_row[row].w, s_bg, kq ? kq + it * 128 : nullptr, wtab, pc + it * 128,
+                                 pi + it * 128, pd + it * 128, pr ? pr + it * 128 : nullptr, HW);
                 }
-                const size_t o = (size_t)row * W + col;
-                *reinterpret_cast<uint32_t *>(pc + o) = cls4;
-                *reinterpret_cast<int4 *>(pi + o) = inst4;
-                *reinterpret_cast<float4 *>(pd + o) = dep4;
-                if (pr) {
-                    *reinterpret_cast<uint32_t *>(pr + o) = r4;
-                    *reinterpret_cast<uint32_t *>(pr + HW + o) = g4;
-                    *reinterpret_cast<uint32_t *>(pr + 2 * HW + o) = b4;
+            } else {
+                int row = row0 + lane_row, col = lane_col, off = 0;
+                while (row <= row1) {
+                    resolve_quad(s_row[row].w, s_bg, kq ? kq + off : nullptr, wtab, pc + off, pi + off, pd + off,
+                                 pr ? pr + off : nullptr, HW);
+                    off += 128; row += step_row; col += step_col;
+                    if (col >= W) { col -= W; ++row; }
                 }
-                row += step_row; col += step_col;
-                if (col >= W) { col -= W; ++row; }
             }
         }
         __syncwarp();      // the key buffer is reused by this warp's next strip

@@ -11,7 +11,7 @@ __device__ __forceinline__ void write_meta(const gp_prim &p, PrimMeta *out, cons
     float qy = c_fma(p.cos_yaw, sc.Ly, -c_mul(p.sin_yaw, sc.Lx));
     float q[3] = {qx, qy, sc.Lz};
     PrimMeta m;
-    m.inst = p.inst; m.pad = 0;
+    m.inst = p.inst; m.inst_dup = p.inst;
     const uint32_t c = (uint32_t)p.cls & 3u;
 #pragma unroll
     for (int a = 0; a < 3; ++a) {

@@ -291,20 +291,27 @@ static int render_device(gp_ctx *c, int world_begin, int n_worlds, int H, int W,
     const int LR = SR < 4 ? SR : 4;
     ra.log2LC = LR == 4 ? 3 : LR == 2 ? 4 : 5;
     ra.o_cls = d_class; ra.o_inst = d_instance; ra.o_depth = d_depth; ra.o_rgb = d_rgb; ra.stats = stats;
+    int log2W = 0;
+    while ((1 << log2W) < W) ++log2W;
+    ra.log2W = log2W;
+    const bool fast4 = (1 << log2W) == W && SR * W == 512 && H % SR == 0;
     const int n_strips = (H + SR - 1) / SR;
     const int nwarps = n_strips < 8 ? n_strips : 8;
-    const size_t smem = 16 + (size_t)ra.cap * 64 + (size_t)H * 16 + (size_t)((W + 3) & ~3) * 4 +
+    const size_t smem = 48 + (size_t)ra.cap * 64 + (size_t)H * 16 + (size_t)((W + 3) & ~3) * 4 +
                         (size_t)nwarps * SR * W * 8;
     if (smem > 227 * 1024) return GP_ERR_ARG;
     if (smem > c->render_smem_set) {
-        CK(cudaFuncSetAttribute(k_render<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        CK(cudaFuncSetAttribute(k_render<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        CK(cudaFuncSetAttribute(k_render<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        CK(cudaFuncSetAttribute(k_render<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        CK(cudaFuncSetAttribute(k_render<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        CK(cudaFuncSetAttribute(k_render<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         c->render_smem_set = smem;
     }
     {
         LaunchTimer lt(c, GP_KERNEL_RENDER, stream);
-        if (stats) k_render<true><<<(unsigned)views, nwarps * 32, smem, stream>>>(sc, ra);
-        else k_render<false><<<(unsigned)views, nwarps * 32, smem, stream>>>(sc, ra);
+        const dim3 g((unsigned)views), b(nwarps * 32);
+        if (stats) { if (fast4) k_render<true, true><<<g, b, smem, stream>>>(sc, ra); else k_render<true, false><<<g, b, smem, stream>>>(sc, ra); }
+        else { if (fast4) k_render<false, true><<<g, b, smem, stream>>>(sc, ra); else k_render<false, false><<<g, b, smem, stream>>>(sc, ra); }
     }
     c->launches += 1;
     CK(cudaGetLastError());
