@@ -34,11 +34,11 @@ k_cull(SceneConst sc, const gp_prim *__restrict__ prims, const float2 *__restric
        int world_begin, int H, int W, float th, float tv,
        ViewHdr *__restrict__ hdr, EntryGeo *__restrict__ geo, EntryAux *__restrict__ aux, int cap,
        unsigned long long *__restrict__ stats) {
-    __shared__ int s_cnt;
+    __shared__ int s_cnt, s_rmin;
     const int view = blockIdx.x;
     const int w = world_begin + view / sc.A, a = view % sc.A;
     const gp_prim *wp = prims + (size_t)w * sc.P;
-    if (threadIdx.x == 0) s_cnt = 0;
+    if (threadIdx.x == 0) { s_cnt = 0; s_rmin = 0x1fff; }
     const float2 pc = __ldg(&pitch[(size_t)w * sc.A + a]);
     const float cp = pc.x, sp = pc.y;
     // C2 camera (contract operations)
@@ -151,6 +151,7 @@ k_cull(SceneConst sc, const gp_prim *__restrict__ prims, const float2 *__restric
             if (c0 > c1 || r0 > r1) continue;                             // touches no pixel centre
         }
         const int slot = atomicAdd(&s_cnt, 1);
+        atomicMin(&s_rmin, r0);
         vgeo[slot] = g;
         EntryAux x;
         x.kf = ((uint32_t)k << 1) | (hz == 0.0f ? 1u : 0u);
@@ -161,7 +162,7 @@ k_cull(SceneConst sc, const gp_prim *__restrict__ prims, const float2 *__restric
     }
     __syncthreads();
     if (threadIdx.x == 0) {
-        ViewHdr h; h.n = s_cnt; h.oz = oz; h.cp = cp; h.sp = sp;
+        ViewHdr h; h.n = s_cnt | (s_rmin << 19); h.oz = oz; h.cp = cp; h.sp = sp;
         hdr[view] = h;
         if (stats) atomicAdd(&stats[1], (unsigned long long)s_cnt);
     }

@@ -94,11 +94,41 @@ __device__ __forceinline__ void resolve_quad(float tg, const uint4 *s_bg, const 
     }
 }
 
+// Contract C5 (per-pixel part) + C6 for one ray against one staged entry: exact fp32 slab test and
+// lexicographic-minimum update of the pixel's key.  g0 = (ax bx ay by), g1 = (az bz . .); dlx, dly are
+// the box-frame direction (already formed with the contract's fma chain), rt = (v, dz, 1/dz, tg).
+__device__ __forceinline__ void slab_select(const float4 &g0, const float4 &g1, float dlx, float dly,
+                                            const float4 &rt, float t_max, bool flat, uint32_t klow,
+                                            unsigned long long *kp) {
+    const float ix = c_rcp(dlx), iy = c_rcp(dly);
+    float ta, tb;
+    ta = c_mul(g0.x, ix); tb = c_mul(g0.y, ix);
+    const float lox = c_min(ta, tb), hix = c_max(ta, tb);
+    ta = c_mul(g0.z, iy); tb = c_mul(g0.w, iy);
+    const float loy = c_min(ta, tb), hiy = c_max(ta, tb);
+    ta = c_mul(g1.x, rt.z); tb = c_mul(g1.y, rt.z);
+    const float loz = c_min(ta, tb), hiz = c_max(ta, tb);
+    const float tn = c_max(c_max(lox, loy), loz);
+    const float tf = c_min(c_min(hix, hiy), hiz);
+    if (tn <= tf && tn > 0.0f && tn <= t_max) {
+        uint32_t face;                                  // m*2 + (sigma > 0)
+        if (flat) face = 5;
+        else if (lox == tn) face = 0 + (dlx > 0.0f ? 0 : 1);
+        else if (loy == tn) face = 2 + (dly > 0.0f ? 0 : 1);
+        else face = 4 + (rt.y > 0.0f ? 0 : 1);
+        const unsigned long long key = ((unsigned long long)__float_as_uint(tn) << 32) | klow | face;   // C6
+        if (key < *kp) *kp = key;
+    }
+}
+
+#ifndef GP_RENDER_WARPS
+#define GP_RENDER_WARPS 4          // warps per CTA (one CTA per view)
+#endif
 #ifndef GP_RENDER_MIN_CTAS
-#define GP_RENDER_MIN_CTAS 4
+#define GP_RENDER_MIN_CTAS (32 / GP_RENDER_WARPS)
 #endif
 template <bool STATS, bool FAST4>
-__global__ void __launch_bounds__(256, GP_RENDER_MIN_CTAS)
+__global__ void __launch_bounds__(GP_RENDER_WARPS * 32, GP_RENDER_MIN_CTAS)
 k_render(SceneConst sc, RenderArgs ra) {
     extern __shared__ __align__(16) unsigned char smem[];
     const int view = blockIdx.x;
@@ -117,7 +147,8 @@ k_render(SceneConst sc, RenderArgs ra) {
 
     const float4 vh4 = __ldg(reinterpret_cast<const float4 *>(&ra.hdr[view]));
     ViewHdr vh; vh.n = __float_as_int(vh4.x); vh.oz = vh4.y; vh.cp = vh4.z; vh.sp = vh4.w;
-    const int n = vh.n;
+    const int n = vh.n & 0x7ffff, rmin = (int)((uint32_t)vh.n >> 19);
+    int *s_next = reinterpret_cast<int *>(smem + 8);               // dynamic strip counter
     if (threadIdx.x == 32 % blockDim.x) {
         const uint32_t g = shade_rgb(sc.pal[1], shade_scale(c_max(sc.Lz, 0.0f), sc.ambient)), k = sc.pal[0];
         s_bg[0] = make_uint4(0u, (k & 0xff) * 0x01010101u, ((k >> 8) & 0xff) * 0x01010101u, ((k >> 16) & 0xff) * 0x01010101u);
@@ -125,6 +156,7 @@ k_render(SceneConst sc, RenderArgs ra) {
                              ((g >> 16) & 0xff) * 0x01010101u);
     }
     if (threadIdx.x == 0) {
+        *s_next = 0;
         mbar_init(bar, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         if (n > 0) {
@@ -147,7 +179,6 @@ k_render(SceneConst sc, RenderArgs ra) {
         s_row[i] = make_float4(v, dz, inv_z, tg);
     }
     __syncthreads();                       // tables + mbarrier init visible
-    if (n > 0) mbar_wait(bar, 0);
 
     const int w = ra.world_begin + view / sc.A;
     const uint32_t *wtab = reinterpret_cast<const uint32_t *>(ra.meta + (size_t)w * sc.P);   // uint32[P][8]
@@ -161,14 +192,25 @@ k_render(SceneConst sc, RenderArgs ra) {
     const float t_max = sc.t_max;
     unsigned long long n_tests = 0;
 
-    for (int strip = warp; strip < n_strips; strip += nwarps) {
+    // Strip schedule: strips are handed out dynamically in ascending order (ascending addresses are
+    // also what the HBM likes: a descending order measured 13% slower).  Strips wholly above the first
+    // row any entry touches need no list and are rendered while the bulk copies are still in flight.
+    const int n_free = n > 0 ? min(n_strips, rmin / SR) : n_strips;
+    bool list_ready = false;
+    for (;;) {
+        int strip = 0;
+        if (lane == 0) strip = atomicAdd(s_next, 1);
+        strip = __shfl_sync(0xffffffffu, strip, 0);
+        if (strip >= n_strips) break;
+        if (strip >= n_free && !list_ready) { mbar_wait(bar, 0); list_ready = true; }
+        const int nn = strip < n_free ? 0 : n;                      // entries to scan for this strip
         const int row0 = strip * SR, row1 = min(H, row0 + SR) - 1;
         bool any = false;
         // ---- a3: warp-level early-out over the list, a6/a7: slab test + select ----------------
-        for (int base = 0; base < n; base += 32) {
+        for (int base = 0; base < nn; base += 32) {
             const int e = base + lane;
             bool ov = false;
-            if (e < n) {
+            if (e < nn) {
                 const uint32_t rows = s_aux[e].rows;
                 ov = (int)(rows & 0xffff) <= row1 && (int)(rows >> 16) >= row0;
             }
@@ -196,51 +238,77 @@ k_render(SceneConst sc, RenderArgs ra) {
                 const float mx = 0.5f * (g0.x + g0.y), my = 0.5f * (g0.z + g0.w), mz = 0.5f * (g1.x + g1.y);   // -ol
                 const float ex_ = 0.5f * (g0.y - g0.x), ey_ = 0.5f * (g0.w - g0.z), ez_ = 0.5f * (g1.y - g1.x); // h
                 const float kSlack = 2e-5f, kGrow = 1.00002f;
-                for (int rb = r0; rb <= r1; rb += LR) {
-                    const int i = rb + li;
-                    for (int cb = c0; cb <= c1; cb += LC) {
-                        const int j = cb + lj;
-                        if (i <= r1 && j <= c1) {
-                            if (STATS) ++n_tests;
-                            const float s = s_col[j];
-                            const float4 rt = s_row[i];                     // v, dz, 1/dz, tg
-                            // C5, per-pixel part
-                            const float dlx = c_fma(rt.x, g2.z, c_fma(s, g2.x, g1.z));
-                            const float dly = c_fma(rt.x, g2.w, c_fma(s, g2.y, g1.w));
-                            const float dlz = rt.y;
-                            // a3 early-out per ray: separating-axis test of the LINE o + t d against the box
-                            // (axes d x e_m).  Division-free; the slack keeps it conservative, so a ray it
-                            // rejects can never pass the exact slab test below.
-                            const float adx = fabsf(dlx), ady = fabsf(dly), adz = fabsf(dlz);
-                            const float px_ = my * dlz, qx_ = mz * dly;
-                            const float py_ = mz * dlx, qy_ = mx * dlz;
-                            const float pz_ = mx * dly, qz_ = my * dlx;
-                            const bool sep =
-                                fabsf(px_ - qx_) > fmaf(ey_, adz, ez_ * ady) * kGrow + kSlack * (fabsf(px_) + fabsf(qx_)) + 1e-12f ||
-                                fabsf(py_ - qy_) > fmaf(ez_, adx, ex_ * adz) * kGrow + kSlack * (fabsf(py_) + fabsf(qy_)) + 1e-12f ||
-                                fabsf(pz_ - qz_) > fmaf(ex_, ady, ey_ * adx) * kGrow + kSlack * (fabsf(pz_) + fabsf(qz_)) + 1e-12f;
-                            if (!sep) {
-                                const float ix = c_rcp(dlx), iy = c_rcp(dly);
-                                float ta, tb;
-                                ta = c_mul(g0.x, ix); tb = c_mul(g0.y, ix);
-                                const float lox = c_min(ta, tb), hix = c_max(ta, tb);
-                                ta = c_mul(g0.z, iy); tb = c_mul(g0.w, iy);
-                                const float loy = c_min(ta, tb), hiy = c_max(ta, tb);
-                                ta = c_mul(g1.x, rt.z); tb = c_mul(g1.y, rt.z);
-                                const float loz = c_min(ta, tb), hiz = c_max(ta, tb);
-                                const float tn = c_max(c_max(lox, loy), loz);
-                                const float tf = c_min(c_min(hix, hiy), hiz);
-                                if (tn <= tf && tn > 0.0f && tn <= t_max) {
-                                    uint32_t face;                                  // m*2 + (sigma > 0)
-                                    if (flat) face = 5;
-                                    else if (lox == tn) face = 0 + (dlx > 0.0f ? 0 : 1);
-                                    else if (loy == tn) face = 2 + (dly > 0.0f ? 0 : 1);
-                                    else face = 4 + (dlz > 0.0f ? 0 : 1);
-                                    const unsigned long long key =
-                                        ((unsigned long long)__float_as_uint(tn) << 32) | klow | face;   // C6
-                                    unsigned long long *kp = &keys[(i - row0) * W + j];
-                                    if (key < *kp) *kp = key;
+                if (flat && c1 - c0 >= LC) {
+                    // Wide flat primitive: per row, the plane depth t is fixed, so the footprint is one
+                    // column interval.  Bound it conservatively (plain fp32 + slack) and run the exact
+                    // test only inside it: a thin diagonal marking costs ~its length, not its bbox area.
+                    const float dl_ = 2e-5f * (fabsf(mx) + fabsf(my) + fabsf(mz) + ex_ + ey_) + 1e-6f;
+                    const float hxs = ex_ + dl_, hys = ey_ + dl_;
+                    const float col_scale = 0.5f * (float)W / ra.th;
+                    for (int rb = r0; rb <= r1; rb += LR) {
+                        const int i = rb + li;
+                        int ja = 1, jb = 0;                                  // empty
+                        float4 rt = make_float4(0.f, 0.f, 0.f, 0.f);
+                        if (i <= r1) {
+                            rt = s_row[i];
+                            const float t = g1.x * rt.z;                     // plane depth on this row
+                            if (t > 0.0f && t <= t_max * 1.00001f) {
+                                const float X0 = fmaf(t, fmaf(rt.x, g2.z, g1.z), -mx), X1 = t * g2.x;
+                                const float Y0 = fmaf(t, fmaf(rt.x, g2.w, g1.w), -my), Y1 = t * g2.y;
+                                float slo = -3.0e38f, shi = 3.0e38f;
+                                bool ok = true;
+                                if (fabsf(X1) > 1e-12f) {
+                                    const float r = 1.0f / X1, a = (-hxs - X0) * r, b = (hxs - X0) * r;
+                                    slo = fmaxf(slo, fminf(a, b)); shi = fminf(shi, fmaxf(a, b));
+                                } else ok = fabsf(X0) <= hxs;
+                                if (fabsf(Y1) > 1e-12f) {
+                                    const float r = 1.0f / Y1, a = (-hys - Y0) * r, b = (hys - Y0) * r;
+                                    slo = fmaxf(slo, fminf(a, b)); shi = fminf(shi, fmaxf(a, b));
+                                } else ok = ok && fabsf(Y0) <= hys;
+                                if (ok && slo <= shi) {
+                                    // column of s: (s/th + 1) W/2 - 0.5, widened by 0.02 px + relative slack
+                                    const float xa = fmaf(slo, col_scale, 0.5f * (float)W - 0.52f) - 1e-5f * fabsf(slo * col_scale);
+                                    const float xb = fmaf(shi, col_scale, 0.5f * (float)W - 0.48f) + 1e-5f * fabsf(shi * col_scale);
+                                    ja = max(c0, (int)ceilf(fmaxf(xa, -1.0f)));
+                                    jb = min(c1, (int)floorf(fminf(xb, (float)W)));
                                 }
+                            }
+                        }
+                        for (int j = ja + lj; __any_sync(0xffffffffu, j <= jb); j += LC) {
+                            if (j <= jb) {
+                                if (STATS) ++n_tests;
+                                const float s = s_col[j];
+                                const float dlx = c_fma(rt.x, g2.z, c_fma(s, g2.x, g1.z));
+                                const float dly = c_fma(rt.x, g2.w, c_fma(s, g2.y, g1.w));
+                                slab_select(g0, g1, dlx, dly, rt, t_max, true, klow, &keys[(i - row0) * W + j]);
+                            }
+                        }
+                    }
+                } else {
+                    for (int rb = r0; rb <= r1; rb += LR) {
+                        const int i = rb + li;
+                        for (int cb = c0; cb <= c1; cb += LC) {
+                            const int j = cb + lj;
+                            if (i <= r1 && j <= c1) {
+                                if (STATS) ++n_tests;
+                                const float s = s_col[j];
+                                const float4 rt = s_row[i];                     // v, dz, 1/dz, tg
+                                // C5, per-pixel part
+                                const float dlx = c_fma(rt.x, g2.z, c_fma(s, g2.x, g1.z));
+                                const float dly = c_fma(rt.x, g2.w, c_fma(s, g2.y, g1.w));
+                                const float dlz = rt.y;
+                                // a3 early-out per ray: separating-axis test of the LINE o + t d against the
+                                // box (axes d x e_m).  Division-free; the slack keeps it conservative, so a
+                                // ray it rejects can never pass the exact slab test.
+                                const float adx = fabsf(dlx), ady = fabsf(dly), adz = fabsf(dlz);
+                                const float px_ = my * dlz, qx_ = mz * dly;
+                                const float py_ = mz * dlx, qy_ = mx * dlz;
+                                const float pz_ = mx * dly, qz_ = my * dlx;
+                                const bool sep =
+                                    fabsf(px_ - qx_) > fmaf(ey_, adz, ez_ * ady) * kGrow + kSlack * (fabsf(px_) + fabsf(qx_)) + 1e-12f ||
+                                    fabsf(py_ - qy_) > fmaf(ez_, adx, ex_ * adz) * kGrow + kSlack * (fabsf(py_) + fabsf(qy_)) + 1e-12f ||
+                                    fabsf(pz_ - qz_) > fmaf(ex_, ady, ey_ * adx) * kGrow + kSlack * (fabsf(pz_) + fabsf(qz_)) + 1e-12f;
+                                if (!sep) slab_select(g0, g1, dlx, dly, rt, t_max, flat, klow, &keys[(i - row0) * W + j]);
                             }
                         }
                     }

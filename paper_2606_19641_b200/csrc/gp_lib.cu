@@ -146,7 +146,7 @@ extern "C" int gp_scene_upload(gp_ctx *c, const gp_scene_desc *d, const gp_prim 
     if (d->quads_per_world > 0 && !h_quads) return GP_ERR_ARG;
     if (!(d->cam_height > 0.0f) || !(d->t_max > 0.0f) || !(d->ambient >= 0.0f && d->ambient <= 1.0f)) return GP_ERR_ARG;
     const long long P = (long long)d->agents_per_world + d->quads_per_world;
-    if (P > (1 << 20) || (long long)d->n_worlds * P > (1ll << 31)) return GP_ERR_ARG;
+    if (P >= (1 << 19) || (long long)d->n_worlds * P > (1ll << 31)) return GP_ERR_ARG;
     const size_t Wn = d->n_worlds, A = d->agents_per_world, Q = d->quads_per_world, n = Wn * (size_t)P;
     for (size_t i = 0; i < Wn * A; ++i) {
         const gp_prim &p = h_agents[i];
@@ -296,7 +296,7 @@ static int render_device(gp_ctx *c, int world_begin, int n_worlds, int H, int W,
     ra.log2W = log2W;
     const bool fast4 = (1 << log2W) == W && SR * W == 512 && H % SR == 0;
     const int n_strips = (H + SR - 1) / SR;
-    const int nwarps = n_strips < 8 ? n_strips : 8;
+    const int nwarps = n_strips < GP_RENDER_WARPS ? n_strips : GP_RENDER_WARPS;
     const size_t smem = 48 + (size_t)ra.cap * 64 + (size_t)H * 16 + (size_t)((W + 3) & ~3) * 4 +
                         (size_t)nwarps * SR * W * 8;
     if (smem > 227 * 1024) return GP_ERR_ARG;
