@@ -18,7 +18,7 @@ namespace gp {
 
 struct RenderArgs {
     const ViewHdr *hdr; const EntryGeo *geo; const EntryAux *aux; const PrimMeta *meta;
-    int cap, world_begin, H, W;
+    int cap, scap, world_begin, H, W;   // cap: list stride in global memory; scap: staged capacity
     float th, tv;
     int SR, log2LC;                 // rows per strip; lanes per row of the test tile (LC = 1 << log2LC)
     int log2W;                      // valid when the FAST4 resolve is used (W a power of two)
@@ -139,8 +139,8 @@ k_render(SceneConst sc, RenderArgs ra) {
     uint64_t *bar = reinterpret_cast<uint64_t *>(smem);
     uint4 *s_bg = reinterpret_cast<uint4 *>(smem + 16);            // [0] sky, [1] ground: cls4, r4, g4, b4
     EntryGeo *s_geo = reinterpret_cast<EntryGeo *>(smem + 48);
-    EntryAux *s_aux = reinterpret_cast<EntryAux *>(smem + 48 + (size_t)ra.cap * 48);
-    float4 *s_row = reinterpret_cast<float4 *>(smem + 48 + (size_t)ra.cap * 64);
+    EntryAux *s_aux = reinterpret_cast<EntryAux *>(smem + 48 + (size_t)ra.scap * 48);
+    float4 *s_row = reinterpret_cast<float4 *>(smem + 48 + (size_t)ra.scap * 64);
     float *s_col = reinterpret_cast<float *>(s_row + H);
     unsigned long long *s_keys = reinterpret_cast<unsigned long long *>(s_col + ((W + 3) & ~3));
     unsigned long long *keys = s_keys + (size_t)warp * SR * W;
@@ -160,9 +160,10 @@ k_render(SceneConst sc, RenderArgs ra) {
         mbar_init(bar, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         if (n > 0) {
-            mbar_expect_tx(bar, (uint32_t)n * 64u);
-            bulk_g2s(s_geo, ra.geo + (size_t)view * ra.cap, (uint32_t)n * 48u, bar);
-            bulk_g2s(s_aux, ra.aux + (size_t)view * ra.cap, (uint32_t)n * 16u, bar);
+            const uint32_t ns = (uint32_t)min(n, ra.scap);   // entries beyond scap are read from global memory
+            mbar_expect_tx(bar, ns * 64u);
+            bulk_g2s(s_geo, ra.geo + (size_t)view * ra.cap, ns * 48u, bar);
+            bulk_g2s(s_aux, ra.aux + (size_t)view * ra.cap, ns * 16u, bar);
         }
     }
     // tables (contract C2-C4), overlapped with the bulk copies
@@ -196,6 +197,8 @@ k_render(SceneConst sc, RenderArgs ra) {
     // also what the HBM likes: a descending order measured 13% slower).  Strips wholly above the first
     // row any entry touches need no list and are rendered while the bulk copies are still in flight.
     const int n_free = n > 0 ? min(n_strips, rmin / SR) : n_strips;
+    const EntryGeo *g_geo = ra.geo + (size_t)view * ra.cap;
+    const EntryAux *g_aux = ra.aux + (size_t)view * ra.cap;
     bool list_ready = false;
     for (;;) {
         int strip = 0;
@@ -211,7 +214,7 @@ k_render(SceneConst sc, RenderArgs ra) {
             const int e = base + lane;
             bool ov = false;
             if (e < nn) {
-                const uint32_t rows = s_aux[e].rows;
+                const uint32_t rows = e < ra.scap ? s_aux[e].rows : __ldg(&g_aux[e].rows);
                 ov = (int)(rows & 0xffff) <= row1 && (int)(rows >> 16) >= row0;
             }
             unsigned mask = __ballot_sync(0xffffffffu, ov);
@@ -225,10 +228,16 @@ k_render(SceneConst sc, RenderArgs ra) {
             while (mask) {
                 const int eb = base + __ffs(mask) - 1;
                 mask &= mask - 1;
-                const float4 g0 = *reinterpret_cast<const float4 *>(&s_geo[eb]);          // ax bx ay by
-                const float4 g1 = *(reinterpret_cast<const float4 *>(&s_geo[eb]) + 1);    // az bz flx fly
-                const float4 g2 = *(reinterpret_cast<const float4 *>(&s_geo[eb]) + 2);    // rlx rly ulx uly
-                const uint4 ax = *reinterpret_cast<const uint4 *>(&s_aux[eb]);
+                float4 g0, g1, g2; uint4 ax;        // (ax bx ay by) (az bz flx fly) (rlx rly ulx uly) aux
+                if (eb < ra.scap) {
+                    const float4 *sg = reinterpret_cast<const float4 *>(&s_geo[eb]);
+                    g0 = sg[0]; g1 = sg[1]; g2 = sg[2];
+                    ax = *reinterpret_cast<const uint4 *>(&s_aux[eb]);
+                } else {                            // rare: list longer than the staged capacity
+                    const float4 *gg = reinterpret_cast<const float4 *>(&g_geo[eb]);
+                    g0 = __ldg(gg); g1 = __ldg(gg + 1); g2 = __ldg(gg + 2);
+                    ax = __ldg(reinterpret_cast<const uint4 *>(&g_aux[eb]));
+                }
                 const bool flat = ax.x & 1u;
                 const uint32_t klow = (ax.x >> 1) << 3;
                 const int r0 = max((int)(ax.y & 0xffff), row0), r1 = min((int)(ax.y >> 16), row1);

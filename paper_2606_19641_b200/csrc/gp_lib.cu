@@ -13,6 +13,10 @@
 
 using namespace gp;
 
+#ifndef GP_STAGE_CAP
+#define GP_STAGE_CAP 128
+#endif
+
 struct gp_ctx {
     int device = -1;
     bool have_scene = false;
@@ -25,7 +29,7 @@ struct gp_ctx {
     ViewHdr *d_hdr = nullptr; EntryGeo *d_geo = nullptr; EntryAux *d_aux = nullptr;
     size_t scratch_views = 0; int scratch_cap = 0;
     unsigned long long *d_stats = nullptr;
-    int opt_path = GP_PATH_FAST, opt_stats = 0, opt_timing = 0;
+    int opt_path = GP_PATH_FAST, opt_stats = 0, opt_timing = 0, opt_stage_cap = GP_STAGE_CAP;
     struct Timed { int kernel; cudaEvent_t a, b; };
     std::vector<Timed> timed;                                    // GP_OPT_TIMING records
     std::vector<cudaEvent_t> ev_pool;
@@ -135,6 +139,9 @@ extern "C" int gp_set_option(gp_ctx *c, int key, int value) {
             c->opt_stats = value ? 1 : 0; return GP_OK;
         case GP_OPT_TIMING:
             c->opt_timing = value ? 1 : 0; return GP_OK;
+        case GP_OPT_STAGE_CAP:
+            if (value < 1) return GP_ERR_ARG;
+            c->opt_stage_cap = value; return GP_OK;
         default: return GP_ERR_ARG;
     }
 }
@@ -284,7 +291,7 @@ static int render_device(gp_ctx *c, int world_begin, int n_worlds, int H, int W,
 
     RenderArgs ra;
     ra.hdr = c->d_hdr; ra.geo = c->d_geo; ra.aux = c->d_aux; ra.meta = c->d_meta;
-    ra.cap = c->scratch_cap; ra.world_begin = world_begin; ra.H = H; ra.W = W; ra.th = th; ra.tv = tv;
+    ra.cap = c->scratch_cap; ra.scap = std::min(c->scratch_cap, c->opt_stage_cap); ra.world_begin = world_begin; ra.H = H; ra.W = W; ra.th = th; ra.tv = tv;
     int SR = 1;                                                    // rows per strip: ~512 pixels, power of two
     while (SR < 16 && SR * 2 * W <= 512) SR *= 2;
     ra.SR = SR;
@@ -297,7 +304,7 @@ static int render_device(gp_ctx *c, int world_begin, int n_worlds, int H, int W,
     const bool fast4 = (1 << log2W) == W && SR * W == 512 && H % SR == 0;
     const int n_strips = (H + SR - 1) / SR;
     const int nwarps = n_strips < GP_RENDER_WARPS ? n_strips : GP_RENDER_WARPS;
-    const size_t smem = 48 + (size_t)ra.cap * 64 + (size_t)H * 16 + (size_t)((W + 3) & ~3) * 4 +
+    const size_t smem = 48 + (size_t)ra.scap * 64 + (size_t)H * 16 + (size_t)((W + 3) & ~3) * 4 +
                         (size_t)nwarps * SR * W * 8;
     if (smem > 227 * 1024) return GP_ERR_ARG;
     if (smem > c->render_smem_set) {
