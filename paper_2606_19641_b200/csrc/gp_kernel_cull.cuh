@@ -29,75 +29,129 @@ __device__ __forceinline__ void bound_point(PixBounds &b, float X, float Y, floa
     b.vmin = fminf(b.vmin, v - dv); b.vmax = fmaxf(b.vmax, v + dv);
 }
 
-__global__ void __launch_bounds__(128)
+// Camera of the view (contract C2) and everything of C5 that depends only on (view, primitive).
+struct CullCam { float ox, oy, oz, fx, fy, rx, ry, ux, uy, cp, sp; };
+struct CullPrim {
+    EntryGeo g; float olx, oly, olz, hx, hy, hz;
+    // conservative camera-frame geometry: centre (Xc, Yc, Zc), half-edge vectors, error bound E
+    float E, Xc, Yc, Zc, Xx, Xy, Xz, Yx, Yy, Zx, Zy, Zz, Xr;
+};
+
+__device__ __forceinline__ void cull_hoist(const gp_prim *__restrict__ wp, int k, const CullCam &c, CullPrim &q) {
+    const float4 p0 = __ldg(reinterpret_cast<const float4 *>(&wp[k]));        // cx cy cz hx
+    const float4 p1 = __ldg(reinterpret_cast<const float4 *>(&wp[k]) + 1);    // hy hz ck sk
+    const float pcx = p0.x, pcy = p0.y, pcz = p0.z, ck = p1.z, sk = p1.w;
+    q.hx = p0.w; q.hy = p1.x; q.hz = p1.y;
+    // ---- contract C5, hoisted part -------------------------------------------------------
+    const float ex = c_sub(c.ox, pcx), ey = c_sub(c.oy, pcy);
+    q.olx = c_fma(sk, ey, c_mul(ck, ex));
+    q.oly = c_fma(ck, ey, -c_mul(sk, ex));
+    q.olz = c_sub(c.oz, pcz);
+    EntryGeo &g = q.g;
+    g.flx = c_fma(sk, c.fy, c_mul(ck, c.fx)); g.fly = c_fma(ck, c.fy, -c_mul(sk, c.fx));
+    g.rlx = c_fma(sk, c.ry, c_mul(ck, c.rx)); g.rly = c_fma(ck, c.ry, -c_mul(sk, c.rx));
+    g.ulx = c_fma(sk, c.uy, c_mul(ck, c.ux)); g.uly = c_fma(ck, c.uy, -c_mul(sk, c.ux));
+    g.ax = c_sub(-q.hx, q.olx); g.bx = c_sub(q.hx, q.olx);
+    g.ay = c_sub(-q.hy, q.oly); g.by = c_sub(q.hy, q.oly);
+    g.az = c_sub(-q.hz, q.olz); g.bz = c_sub(q.hz, q.olz);
+    // ---- conservative geometry (not contract arithmetic) ----------------------------------
+    // Camera coordinates of a box-frame point p: X = (p-ol).f_l (planar depth), Y = (p-ol).r_l
+    // (right), Z = (p-ol).u_l (up), with f_l = (flx, fly, sp), r_l = (rlx, rly, 0), u_l = (ulx, uly, cp).
+    q.E = 1e-5f * (fabsf(q.olx) + fabsf(q.oly) + fabsf(q.olz) + q.hx + q.hy + q.hz) + 1e-6f;
+    q.Xc = -(q.olx * g.flx + q.oly * g.fly + q.olz * c.sp);
+    q.Yc = -(q.olx * g.rlx + q.oly * g.rly);
+    q.Zc = -(q.olx * g.ulx + q.oly * g.uly + q.olz * c.cp);
+    q.Xx = q.hx * g.flx; q.Xy = q.hy * g.fly; q.Xz = q.hz * c.sp;        // half-edge vectors, camera frame
+    q.Yx = q.hx * g.rlx; q.Yy = q.hy * g.rly;
+    q.Zx = q.hx * g.ulx; q.Zy = q.hy * g.uly; q.Zz = q.hz * c.cp;
+    q.Xr = fabsf(q.Xx) + fabsf(q.Xy) + fabsf(q.Xz);
+}
+
+// Phase-1 test: can the box touch the view volume at all?  (near / far / four side planes, exact
+// support function of the box along each plane normal, widened by the error bound.)
+__device__ __forceinline__ bool cull_in_frustum(const CullPrim &q, float th, float tv, float t_max) {
+    const float E = q.E;
+    if (q.Xc + q.Xr < -E) return false;                                   // wholly behind the camera plane
+    if (q.Xc - q.Xr > t_max * (1.0f + 1e-6f) + E) return false;           // wholly beyond the far plane
+    const float m = E * (2.0f + th + tv);
+    float gc, gr;
+    gc = q.Yc - th * q.Xc;  gr = fabsf(q.Yx - th * q.Xx) + fabsf(q.Yy - th * q.Xy) + fabsf(th * q.Xz);
+    if (gc - gr > m) return false;
+    gc = -q.Yc - th * q.Xc; gr = fabsf(q.Yx + th * q.Xx) + fabsf(q.Yy + th * q.Xy) + fabsf(th * q.Xz);
+    if (gc - gr > m) return false;
+    gc = q.Zc - tv * q.Xc;  gr = fabsf(q.Zx - tv * q.Xx) + fabsf(q.Zy - tv * q.Xy) + fabsf(q.Zz - tv * q.Xz);
+    if (gc - gr > m) return false;
+    gc = -q.Zc - tv * q.Xc; gr = fabsf(q.Zx + tv * q.Xx) + fabsf(q.Zy + tv * q.Xy) + fabsf(q.Zz + tv * q.Xz);
+    if (gc - gr > m) return false;
+    return true;
+}
+
+constexpr int kCullChunk = 256;        // primitives per two-phase round
+constexpr int kCullWarps = 4;          // views per CTA: one warp per view, no block-level barrier
+
+__global__ void __launch_bounds__(kCullWarps * 32)
 k_cull(SceneConst sc, const gp_prim *__restrict__ prims, const float2 *__restrict__ pitch,
-       int world_begin, int H, int W, float th, float tv,
+       int world_begin, int n_views, int H, int W, float th, float tv,
        ViewHdr *__restrict__ hdr, EntryGeo *__restrict__ geo, EntryAux *__restrict__ aux, int cap,
        unsigned long long *__restrict__ stats) {
-    __shared__ int s_cnt, s_rmin;
-    const int view = blockIdx.x;
+    __shared__ int s_idx_all[kCullWarps][kCullChunk];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int view = blockIdx.x * kCullWarps + warp;
+    if (view >= n_views) return;
+    int *s_idx = s_idx_all[warp];
+    const unsigned lt_mask = (1u << lane) - 1u;
     const int w = world_begin + view / sc.A, a = view % sc.A;
     const gp_prim *wp = prims + (size_t)w * sc.P;
-    if (threadIdx.x == 0) { s_cnt = 0; s_rmin = 0x1fff; }
     const float2 pc = __ldg(&pitch[(size_t)w * sc.A + a]);
-    const float cp = pc.x, sp = pc.y;
+    CullCam cam;
+    cam.cp = pc.x; cam.sp = pc.y;
     // C2 camera (contract operations)
-    const float e_hx = __ldg(&wp[a].hx), e_ck = __ldg(&wp[a].cos_yaw), e_sk = __ldg(&wp[a].sin_yaw);
-    const float ox = c_fma(e_hx, e_ck, __ldg(&wp[a].cx)), oy = c_fma(e_hx, e_sk, __ldg(&wp[a].cy));
-    const float oz = sc.cam_h;
-    const float fx = c_mul(cp, e_ck), fy = c_mul(cp, e_sk);
-    const float rx = e_sk, ry = -e_ck;
-    const float ux = -c_mul(sp, e_ck), uy = -c_mul(sp, e_sk);
-    __syncthreads();
+    const float4 e0 = __ldg(reinterpret_cast<const float4 *>(&wp[a]));        // cx cy cz hx
+    const float4 e1 = __ldg(reinterpret_cast<const float4 *>(&wp[a]) + 1);    // hy hz ck sk
+    const float e_hx = e0.w, e_ck = e1.z, e_sk = e1.w;
+    cam.ox = c_fma(e_hx, e_ck, e0.x); cam.oy = c_fma(e_hx, e_sk, e0.y);
+    cam.oz = sc.cam_h;
+    cam.fx = c_mul(cam.cp, e_ck); cam.fy = c_mul(cam.cp, e_sk);
+    cam.rx = e_sk; cam.ry = -e_ck;
+    cam.ux = -c_mul(cam.sp, e_ck); cam.uy = -c_mul(cam.sp, e_sk);
 
     EntryGeo *vgeo = geo + (size_t)view * cap;
     EntryAux *vaux = aux + (size_t)view * cap;
     const float halfW = 0.5f * (float)W, halfH = 0.5f * (float)H;
     const float inv_th = 1.0f / th, inv_tv = 1.0f / tv;
+    int cnt = 0, rmin = 0x1fff;            // list length (warp-uniform), first row touched (per lane)
 
-    for (int k = threadIdx.x; k < sc.P; k += blockDim.x) {
-        if (k == a) continue;
-        const float4 p0 = __ldg(reinterpret_cast<const float4 *>(&wp[k]));        // cx cy cz hx
-        const float4 p1 = __ldg(reinterpret_cast<const float4 *>(&wp[k]) + 1);    // hy hz ck sk
-        const float pcx = p0.x, pcy = p0.y, pcz = p0.z, hx = p0.w, hy = p1.x, hz = p1.y, ck = p1.z, sk = p1.w;
-        // ---- contract C5, hoisted part -------------------------------------------------------
-        const float ex = c_sub(ox, pcx), ey = c_sub(oy, pcy);
-        const float olx = c_fma(sk, ey, c_mul(ck, ex));
-        const float oly = c_fma(ck, ey, -c_mul(sk, ex));
-        const float olz = c_sub(oz, pcz);
-        EntryGeo g;
-        g.flx = c_fma(sk, fy, c_mul(ck, fx)); g.fly = c_fma(ck, fy, -c_mul(sk, fx));
-        g.rlx = c_fma(sk, ry, c_mul(ck, rx)); g.rly = c_fma(ck, ry, -c_mul(sk, rx));
-        g.ulx = c_fma(sk, uy, c_mul(ck, ux)); g.uly = c_fma(ck, uy, -c_mul(sk, ux));
-        g.ax = c_sub(-hx, olx); g.bx = c_sub(hx, olx);
-        g.ay = c_sub(-hy, oly); g.by = c_sub(hy, oly);
-        g.az = c_sub(-hz, olz); g.bz = c_sub(hz, olz);
-
-        // ---- conservative geometry (not contract arithmetic) ----------------------------------
-        // Camera coordinates of a box-frame point q: X = (q-ol).f_l (planar depth), Y = (q-ol).r_l
-        // (right), Z = (q-ol).u_l (up), with f_l = (flx, fly, sp), r_l = (rlx, rly, 0), u_l = (ulx, uly, cp).
-        const float E = 1e-5f * (fabsf(olx) + fabsf(oly) + fabsf(olz) + hx + hy + hz) + 1e-6f;
-        const float Xc = -(olx * g.flx + oly * g.fly + olz * sp);
-        const float Yc = -(olx * g.rlx + oly * g.rly);
-        const float Zc = -(olx * g.ulx + oly * g.uly + olz * cp);
-        const float Xx = hx * g.flx, Xy = hy * g.fly, Xz = hz * sp;        // half-edge vectors, camera frame
-        const float Yx = hx * g.rlx, Yy = hy * g.rly;
-        const float Zx = hx * g.ulx, Zy = hy * g.uly, Zz = hz * cp;
-        const float Xr = fabsf(Xx) + fabsf(Xy) + fabsf(Xz);
-        if (Xc + Xr < -E) continue;                                       // wholly behind the camera plane
-        if (Xc - Xr > sc.t_max * (1.0f + 1e-6f) + E) continue;            // wholly beyond the far plane
-        {   // support test against the four side planes  +-Y - th X <= 0,  +-Z - tv X <= 0
-            const float m = E * (2.0f + th + tv);
-            float gc, gr;
-            gc = Yc - th * Xc;  gr = fabsf(Yx - th * Xx) + fabsf(Yy - th * Xy) + fabsf(th * Xz);
-            if (gc - gr > m) continue;
-            gc = -Yc - th * Xc; gr = fabsf(Yx + th * Xx) + fabsf(Yy + th * Xy) + fabsf(th * Xz);
-            if (gc - gr > m) continue;
-            gc = Zc - tv * Xc;  gr = fabsf(Zx - tv * Xx) + fabsf(Zy - tv * Xy) + fabsf(Zz - tv * Xz);
-            if (gc - gr > m) continue;
-            gc = -Zc - tv * Xc; gr = fabsf(Zx + tv * Xx) + fabsf(Zy + tv * Xy) + fabsf(Zz + tv * Xz);
-            if (gc - gr > m) continue;
+    for (int k0 = 0; k0 < sc.P; k0 += kCullChunk) {
+        // ---- phase 1: one primitive per lane: frustum test, survivors compacted (ballot) into s_idx
+        const int k1 = min(sc.P, k0 + kCullChunk);
+        int m = 0;
+        for (int kb = k0; kb < k1; kb += 32) {
+            const int k = kb + lane;
+            bool pass = false;
+            if (k < k1 && k != a) {
+                CullPrim q;
+                cull_hoist(wp, k, cam, q);
+                pass = cull_in_frustum(q, th, tv, sc.t_max);
+            }
+            const unsigned mask = __ballot_sync(0xffffffffu, pass);
+            if (pass) s_idx[m + __popc(mask & lt_mask)] = k;
+            m += __popc(mask);
         }
+        __syncwarp();
+        // ---- phase 2: dense over the survivors: pixel bounds by corner projection, list append
+        for (int ib = 0; ib < m; ib += 32) {
+        const int it = ib + lane;
+        bool keep = false;
+        EntryGeo g; EntryAux x;
+        if (it < m) {
+        const int k = s_idx[it];
+        CullPrim q;
+        cull_hoist(wp, k, cam, q);
+        g = q.g;
+        const float E = q.E, Xc = q.Xc, Yc = q.Yc, Zc = q.Zc, Xr = q.Xr;
+        const float Xx = q.Xx, Xy = q.Xy, Xz = q.Xz, Yx = q.Yx, Yy = q.Yy, Zx = q.Zx, Zy = q.Zy, Zz = q.Zz;
+        const float hz = q.hz;
+        keep = true;
         // corner projection with near-plane clipping
         float cX[8], cY[8], cZ[8];
 #pragma unroll
@@ -148,23 +202,29 @@ k_cull(SceneConst sc, const gp_prim *__restrict__ prims, const float2 *__restric
             const float yh = fminf(fmaxf((1.0f - b.vmin * inv_tv) * halfH - 0.48f, -1.0f), (float)H);
             c0 = max((int)ceilf(xl), 0); c1 = min((int)floorf(xh), W - 1);
             r0 = max((int)ceilf(yl), 0); r1 = min((int)floorf(yh), H - 1);
-            if (c0 > c1 || r0 > r1) continue;                             // touches no pixel centre
+            if (c0 > c1 || r0 > r1) keep = false;                         // touches no pixel centre
         }
-        const int slot = atomicAdd(&s_cnt, 1);
-        atomicMin(&s_rmin, r0);
-        vgeo[slot] = g;
-        EntryAux x;
+        if (keep) rmin = min(rmin, r0);
         x.kf = ((uint32_t)k << 1) | (hz == 0.0f ? 1u : 0u);
         x.rows = (uint32_t)r0 | ((uint32_t)r1 << 16);
         x.cols = (uint32_t)c0 | ((uint32_t)c1 << 16);
         x.pad = 0;
-        vaux[slot] = x;
+        }
+        const unsigned kmask = __ballot_sync(0xffffffffu, keep);
+        if (keep) {
+            const int slot = cnt + __popc(kmask & lt_mask);
+            vgeo[slot] = g;
+            vaux[slot] = x;
+        }
+        cnt += __popc(kmask);
+        }
+        __syncwarp();
     }
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        ViewHdr h; h.n = s_cnt | (s_rmin << 19); h.oz = oz; h.cp = cp; h.sp = sp;
+    rmin = __reduce_min_sync(0xffffffffu, rmin);
+    if (lane == 0) {
+        ViewHdr h; h.n = cnt | (rmin << 19); h.oz = cam.oz; h.cp = cam.cp; h.sp = cam.sp;
         hdr[view] = h;
-        if (stats) atomicAdd(&stats[1], (unsigned long long)s_cnt);
+        if (stats) atomicAdd(&stats[1], (unsigned long long)cnt);
     }
 }
 
