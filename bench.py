@@ -288,10 +288,12 @@ def run_b200(args):
     r_avg_ms = r_ms / max(1, r_n)
     achieved = alg_bytes / (r_avg_ms * 1e-3) / 1e9
     traffic = None
-    tpath = os.path.join(ROOT, "profiles", "traffic.json")
-    if os.path.exists(tpath):
-        with open(tpath) as f:
-            traffic = json.load(f).get(cfg.name)
+    tpath = os.path.join(ROOT, "profiles", "r01_traffic.txt")      # from the committed ncu --set full capture
+    if os.path.exists(tpath) and not args.worlds and not args.res:
+        for line in open(tpath):
+            part = line.split()
+            if len(part) == 2 and part[0] == cfg.name:
+                traffic = int(part[1])
     sm_mhz = (clocks or {}).get("sm_mhz") or 1965.0
     fp32_peak = 148 * 128 * 2 * sm_mhz * 1e6
     t_fp32_ms = stats["executed_tests"] * FP32_OPS_PER_TEST / fp32_peak * 1e3
@@ -319,7 +321,7 @@ def run_b200(args):
     if not args.no_cpu_baseline and world_size == 1:
         threads = max(1, min(64, os.cpu_count() or 1))
         per_core_s = 0.09 * (cfg.H * cfg.W * cfg.prims) / (128 * 128 * 264)
-        n_views = int(min(cfg.views, max(threads, round(12.0 * threads / per_core_s))))
+        n_views = int(min(cfg.views, max(threads, round(40.0 * threads / per_core_s))))
         sec = oracle_sample(cfg, n_views, threads)
         out["cpu_baseline"] = {"value": n_views / sec, "unit": UNIT, "cores": threads, "kind": "oracle",
                                "sample": "%d views of the workload (frame 0), all-primitive fp32 oracle (oracle/gp_oracle.c), %d threads, %.1f s"
