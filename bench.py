@@ -147,9 +147,11 @@ def run_reference(args):
     cfg = workload_cfg(args)
     threads = max(1, min(64, os.cpu_count() or 1))
     per_core_s = 0.09 * (cfg.H * cfg.W * cfg.prims) / (128 * 128 * 264)
-    n_views = max(threads, int(min(cfg.views, max(1, round(6.0 * threads / per_core_s)))))   # ~6 s per step
+    # bounded sample: the whole --steps/--warmup run should end within ~2.5 minutes
+    step_s = min(20.0, max(0.2, 150.0 / max(1, args.steps + args.warmup)))
+    n_views = max(threads, int(min(cfg.views, max(1, round(step_s * threads / per_core_s)))))
     for _ in range(args.warmup):
-        oracle_sample(cfg, min(n_views, threads), threads)
+        oracle_sample(cfg, n_views, threads)
     t = [oracle_sample(cfg, n_views, threads) for _ in range(args.steps)]
     total = sum(t)
     value = n_views * args.steps / total
