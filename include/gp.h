@@ -44,8 +44,9 @@ enum {
     GP_OPT_PATH = 1,        /* GP_PATH_FAST (default) or GP_PATH_BRUTE                        */
     GP_OPT_STATS = 2,       /* 1: count executed ray/primitive tests and listed pairs         */
     GP_OPT_TIMING = 3,      /* 1: bracket every kernel launch with CUDA events (gp_kernel_time) */
-    GP_OPT_STAGE_CAP = 4    /* list entries per view staged in shared memory (default 128, >= 1);
+    GP_OPT_STAGE_CAP = 4,   /* list entries per view staged in shared memory (default 128, >= 1);
                                longer lists read their tail from global memory                  */
+    GP_OPT_STRIP_PX = 5     /* target pixels per warp strip of the render pass; 0 = automatic   */
 };
 enum {                      /* kernel ids of gp_kernel_time                                   */
     GP_KERNEL_UPDATE = 0,   /* a0 pose update + shading table                                 */

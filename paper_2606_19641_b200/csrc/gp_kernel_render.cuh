@@ -21,7 +21,7 @@ struct RenderArgs {
     int cap, scap, world_begin, H, W;   // cap: list stride in global memory; scap: staged capacity
     float th, tv;
     int SR, log2LC;                 // rows per strip; lanes per row of the test tile (LC = 1 << log2LC)
-    int log2W;                      // valid when the FAST4 resolve is used (W a power of two)
+    int log2W;                      // valid when NG > 0 (W a power of two)
     uint8_t *o_cls; int32_t *o_inst; float *o_depth; uint8_t *o_rgb;
     unsigned long long *stats;
 };
@@ -127,7 +127,7 @@ __device__ __forceinline__ void slab_select(const float4 &g0, const float4 &g1, 
 #ifndef GP_RENDER_MIN_CTAS
 #define GP_RENDER_MIN_CTAS (32 / GP_RENDER_WARPS)
 #endif
-template <bool STATS, bool FAST4>
+template <bool STATS, int NG>     // NG: 128-pixel groups per strip when W is a power of two (1, 2, 4), else 0
 __global__ void __launch_bounds__(GP_RENDER_WARPS * 32, GP_RENDER_MIN_CTAS)
 k_render(SceneConst sc, RenderArgs ra) {
     extern __shared__ __align__(16) unsigned char smem[];
@@ -333,9 +333,9 @@ k_render(SceneConst sc, RenderArgs ra) {
             float *pd = ra.o_depth + o0;
             uint8_t *pr = ra.o_rgb ? ra.o_rgb + 2 * (size_t)view * HW + o0 : nullptr;
             const unsigned long long *kq = any ? keys + lane * 4 : nullptr;
-            if (FAST4) {        // strip = 512 pixels = 4 groups, W a power of two: constant offsets
+            if (NG > 0) {       // strip = NG groups of 128 pixels, W a power of two: constant offsets
 #pragma unroll
-                for (int it = 0; it < 4; ++it) {
+                for (int it = 0; it < NG; ++it) {
                     const int row = row0 + ((lane * 4 + it * 128) >> ra.log2W);
                     resolve_quad(s_row[row].w, s_bg, kq ? kq + it * 128 : nullptr, wtab, pc + it * 128,
                                  pi + it * 128, pd + it * 128, pr ? pr + it * 128 : nullptr, HW);

@@ -29,7 +29,7 @@ struct gp_ctx {
     ViewHdr *d_hdr = nullptr; EntryGeo *d_geo = nullptr; EntryAux *d_aux = nullptr;
     size_t scratch_views = 0; int scratch_cap = 0;
     unsigned long long *d_stats = nullptr;
-    int opt_path = GP_PATH_FAST, opt_stats = 0, opt_timing = 0, opt_stage_cap = GP_STAGE_CAP;
+    int opt_path = GP_PATH_FAST, opt_stats = 0, opt_timing = 0, opt_stage_cap = GP_STAGE_CAP, opt_strip_px = 0;
     struct Timed { int kernel; cudaEvent_t a, b; };
     std::vector<Timed> timed;                                    // GP_OPT_TIMING records
     std::vector<cudaEvent_t> ev_pool;
@@ -142,6 +142,9 @@ extern "C" int gp_set_option(gp_ctx *c, int key, int value) {
         case GP_OPT_STAGE_CAP:
             if (value < 1) return GP_ERR_ARG;
             c->opt_stage_cap = value; return GP_OK;
+        case GP_OPT_STRIP_PX:
+            if (value < 0 || value > 4096) return GP_ERR_ARG;
+            c->opt_strip_px = value; return GP_OK;
         default: return GP_ERR_ARG;
     }
 }
@@ -293,8 +296,12 @@ static int render_device(gp_ctx *c, int world_begin, int n_worlds, int H, int W,
     RenderArgs ra;
     ra.hdr = c->d_hdr; ra.geo = c->d_geo; ra.aux = c->d_aux; ra.meta = c->d_meta;
     ra.cap = c->scratch_cap; ra.scap = std::min(c->scratch_cap, c->opt_stage_cap); ra.world_begin = world_begin; ra.H = H; ra.W = W; ra.th = th; ra.tv = tv;
-    int SR = 1;                                                    // rows per strip: ~512 pixels, power of two
-    while (SR < 16 && SR * 2 * W <= 512) SR *= 2;
+    // rows per strip (power of two): ~512 pixels, fewer for small images so that a view still has
+    // >= 16 strips to spread over its warps (a strip's entries are processed serially by one warp)
+    int strip_px = c->opt_strip_px;
+    if (strip_px <= 0) { strip_px = 512; while (strip_px > 128 && H * W / strip_px < 16) strip_px /= 2; }
+    int SR = 1;
+    while (SR < 16 && SR * 2 * W <= strip_px) SR *= 2;
     ra.SR = SR;
     const int LR = SR < 4 ? SR : 4;
     ra.log2LC = LR == 4 ? 3 : LR == 2 ? 4 : 5;
@@ -302,24 +309,31 @@ static int render_device(gp_ctx *c, int world_begin, int n_worlds, int H, int W,
     int log2W = 0;
     while ((1 << log2W) < W) ++log2W;
     ra.log2W = log2W;
-    const bool fast4 = (1 << log2W) == W && SR * W == 512 && H % SR == 0;
+    int ng = 0;                                                    // unrolled resolve: NG groups of 128 pixels
+    if ((1 << log2W) == W && H % SR == 0 && (SR * W == 128 || SR * W == 256 || SR * W == 512)) ng = SR * W / 128;
     const int n_strips = (H + SR - 1) / SR;
     const int nwarps = n_strips < GP_RENDER_WARPS ? n_strips : GP_RENDER_WARPS;
     const size_t smem = 48 + (size_t)ra.scap * 64 + (size_t)H * 16 + (size_t)((W + 3) & ~3) * 4 +
                         (size_t)nwarps * SR * W * 8;
     if (smem > 227 * 1024) return GP_ERR_ARG;
     if (smem > c->render_smem_set) {
-        CK(cudaFuncSetAttribute(k_render<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        CK(cudaFuncSetAttribute(k_render<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        CK(cudaFuncSetAttribute(k_render<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        CK(cudaFuncSetAttribute(k_render<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        CK(cudaFuncSetAttribute(k_render<false, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        CK(cudaFuncSetAttribute(k_render<false, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        CK(cudaFuncSetAttribute(k_render<false, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        CK(cudaFuncSetAttribute(k_render<false, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        CK(cudaFuncSetAttribute(k_render<true, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        CK(cudaFuncSetAttribute(k_render<true, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        CK(cudaFuncSetAttribute(k_render<true, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        CK(cudaFuncSetAttribute(k_render<true, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         c->render_smem_set = smem;
     }
     {
         LaunchTimer lt(c, GP_KERNEL_RENDER, stream);
         const dim3 g((unsigned)views), b(nwarps * 32);
-        if (stats) { if (fast4) k_render<true, true><<<g, b, smem, stream>>>(sc, ra); else k_render<true, false><<<g, b, smem, stream>>>(sc, ra); }
-        else { if (fast4) k_render<false, true><<<g, b, smem, stream>>>(sc, ra); else k_render<false, false><<<g, b, smem, stream>>>(sc, ra); }
+#define GP_LAUNCH_RENDER(ST, N) k_render<ST, N><<<g, b, smem, stream>>>(sc, ra)
+        if (stats) { if (ng == 4) GP_LAUNCH_RENDER(true, 4); else if (ng == 2) GP_LAUNCH_RENDER(true, 2); else if (ng == 1) GP_LAUNCH_RENDER(true, 1); else GP_LAUNCH_RENDER(true, 0); }
+        else { if (ng == 4) GP_LAUNCH_RENDER(false, 4); else if (ng == 2) GP_LAUNCH_RENDER(false, 2); else if (ng == 1) GP_LAUNCH_RENDER(false, 1); else GP_LAUNCH_RENDER(false, 0); }
+#undef GP_LAUNCH_RENDER
     }
     c->launches += 1;
     CK(cudaGetLastError());
