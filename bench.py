@@ -170,7 +170,7 @@ def run_reference(args):
 def run_b200(args):
     import torch
     import torch.distributed as dist
-    from paper_2606_19641_b200 import Renderer, gp
+    from paper_2606_19641_b200 import Renderer, gp, shard
 
     rank = int(os.environ.get("RANK", "0"))
     world_size = int(os.environ.get("WORLD_SIZE", "1"))
@@ -184,7 +184,7 @@ def run_b200(args):
     cfg = workload_cfg(args)
     # weak scaling: every rank renders its own cfg.n_worlds worlds (rank-disjoint world ids), no collective
     # on the data path (the path has no exchange step: PAPER.md:319).
-    w0 = rank * cfg.n_worlds
+    w0, _ = shard.weak_world_range(rank, cfg.n_worlds)
     agents, quads = gs.gen_world_prims(cfg.replace(n_worlds=w0 + cfg.n_worlds), w0, cfg.n_worlds)
     big = cfg.replace(n_worlds=w0 + cfg.n_worlds)
     speed, yaw_rate = gs.gen_dynamics(big, w0, cfg.n_worlds)
@@ -231,10 +231,7 @@ def run_b200(args):
     ktimes = {name: r.kernel_time(k) for name, k in (("update", gp.GP_KERNEL_UPDATE), ("cull", gp.GP_KERNEL_CULL),
                                                        ("render", gp.GP_KERNEL_RENDER))}
     r.set_option(gp.GP_OPT_TIMING, 0)
-    if distributed:
-        t = torch.tensor([ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms = shard.max_over_ranks(ms, dev)
 
     # one instrumented frame (not timed): executed tests and listed pairs for the FP32 roof
     r.set_option(gp.GP_OPT_STATS, 1)
@@ -263,10 +260,7 @@ def run_b200(args):
                 r.render_batch_host(h_pose[(i + 1) % len(h_pose)], 0, cfg.n_worlds, H, W, fov, *h)   # synchronises
             barrier()
             e_s = time.perf_counter() - t0
-            if distributed:
-                t = torch.tensor([e_s], device=dev, dtype=torch.float64)
-                dist.all_reduce(t, op=dist.ReduceOp.MAX)
-                e_s = float(t.item())
+            e_s = shard.max_over_ranks(e_s, dev)
             e2e = {"value": world_size * cfg.views * args.e2e_steps / e_s, "unit": UNIT,
                    "h2d_bytes_per_step": int(h_pose[0].numel() * 4),
                    "d2h_bytes_per_step": int(sum(x.numel() * x.element_size() for x in h)),
