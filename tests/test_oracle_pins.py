@@ -402,3 +402,16 @@ def test_ties_between_coplanar_quads_go_to_lower_index():
     assert both.any() and (r["inst"][both] == 11).all()
     r2 = oracle.render_view(stack(ego_at_origin(), q2, q1), 0, 64, 64)
     assert (r2["inst"][both] == 22).all()
+
+
+def test_primitive_beats_the_ground_at_equal_depth():
+    # C6: the ground takes k = +inf.  A quad lying exactly in the plane z = 0 has bit-identical depth
+    # (0 - o.z) * (1/d.z) to the ground on every pixel it covers, and must win there.
+    quad = make_prim(12, 0, 0.0, 4.0, 1.5, 0.0, 1, 0, cls=MARK, inst=9)
+    r = oracle.render_view(stack(ego_at_origin(), quad), 0, 64, 64)
+    g = oracle.render_view(stack(ego_at_origin()), 0, 64, 64)
+    covered = r["cls"] == MARK
+    assert covered.sum() > 20
+    assert (r["depth"][covered] == g["depth"][covered]).all()
+    assert (r["t2"][covered] == r["depth"][covered]).all()          # the ground is the tied runner-up
+    assert (r["inst"][covered] == 9).all()
