@@ -1,11 +1,13 @@
-// gp_kernel_cull.cuh — a1 camera setup + a2 frustum cull and compaction (one CTA per view).
+// gp_kernel_cull.cuh — a1 camera setup + a2 frustum cull and compaction (one warp per view, one CTA per
+// group of 8 views of the same world, which share the world's records through shared memory).
 //
 // For every primitive k != ego of the view's world the kernel
 //   1. hoists the (view, primitive) part of contract C5 with the exact contract operations
 //      (EntryGeo: a_m, b_m and the camera basis in the box frame);
 //   2. decides CONSERVATIVELY, with plain fp32 and explicit error margins, whether the box can
-//      touch the view volume (box-vs-frustum-plane support test, near / far), and if so bounds
-//      its projection by a pixel rectangle (corner projection, edges clipped at the near plane);
+//      touch the view volume (first its bounding sphere, then the box-vs-frustum-plane support
+//      test, near / far), and if so bounds its projection by a pixel rectangle (corner
+//      projection, edges clipped at the near plane);
 //   3. appends survivors to the view's list in global memory (EntryGeo 48 B + EntryAux 16 B).
 // Step 2 only ever drops a primitive that cannot produce a contract hit on any pixel centre, and
 // the rectangle contains every pixel it can hit, so the rendered planes are bit-identical to the
@@ -20,11 +22,19 @@ constexpr float kNearGuard = 0.05f;    // cross-section this close to the optica
 
 struct PixBounds { float smin, smax, vmin, vmax; };
 
+// 1/x to ~1 ulp in one MUFU instruction (conservative geometry only; never contract arithmetic)
+__device__ __forceinline__ float rcp_fast(float x) {
+    float r;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+
 __device__ __forceinline__ void bound_point(PixBounds &b, float X, float Y, float Z, float E) {
-    // X >= kNearEps.  (Y +- E(1+|s|)) / X bounds the true s for an absolute coordinate error E.
-    float inv = 1.0f / X;
+    // X >= kNearEps.  (Y +- E(1+|s|)) / X bounds the true s for an absolute coordinate error E; the
+    // 1e-6 relative term covers the approximate reciprocal.
+    float inv = rcp_fast(X);
     float s = Y * inv, v = Z * inv;
-    float ds = E * (1.0f + fabsf(s)) * inv, dv = E * (1.0f + fabsf(v)) * inv;
+    float ds = fmaf(E * (1.0f + fabsf(s)), inv, 1e-6f * fabsf(s)), dv = fmaf(E * (1.0f + fabsf(v)), inv, 1e-6f * fabsf(v));
     b.smin = fminf(b.smin, s - ds); b.smax = fmaxf(b.smax, s + ds);
     b.vmin = fminf(b.vmin, v - dv); b.vmax = fmaxf(b.vmax, v + dv);
 }
@@ -37,9 +47,8 @@ struct CullPrim {
     float E, Xc, Yc, Zc, Xx, Xy, Xz, Yx, Yy, Zx, Zy, Zz, Xr;
 };
 
-__device__ __forceinline__ void cull_hoist(const gp_prim *__restrict__ wp, int k, const CullCam &c, CullPrim &q) {
-    const float4 p0 = __ldg(reinterpret_cast<const float4 *>(&wp[k]));        // cx cy cz hx
-    const float4 p1 = __ldg(reinterpret_cast<const float4 *>(&wp[k]) + 1);    // hy hz ck sk
+__device__ __forceinline__ void cull_hoist(const float4 p0 /* cx cy cz hx */, const float4 p1 /* hy hz ck sk */,
+                                           const CullCam &c, CullPrim &q) {
     const float pcx = p0.x, pcy = p0.y, pcz = p0.z, ck = p1.z, sk = p1.w;
     q.hx = p0.w; q.hy = p1.x; q.hz = p1.y;
     // ---- contract C5, hoisted part -------------------------------------------------------
@@ -86,34 +95,41 @@ __device__ __forceinline__ bool cull_in_frustum(const CullPrim &q, float th, flo
     return true;
 }
 
-constexpr int kCullChunk = 256;        // primitives per two-phase round
-constexpr int kCullWarps = 4;          // views per CTA: one warp per view, no block-level barrier
+constexpr int kCullChunk = 320;        // primitives staged in shared memory per round
+constexpr int kCullWarps = 8;          // views per CTA (one warp per view), all of the same world
 
-__global__ void __launch_bounds__(kCullWarps * 32)
+// Grid: one CTA per (world, group of kCullWarps agents).  The world's records (first 32 bytes of each:
+// centre, half extents, heading) are staged in shared memory once per CTA and shared by its views.
+__global__ void __launch_bounds__(kCullWarps * 32, 3)
 k_cull(SceneConst sc, const gp_prim *__restrict__ prims, const float2 *__restrict__ pitch,
-       int world_begin, int n_views, int H, int W, float th, float tv,
+       int world_begin, int groups_per_world, int H, int W, float th, float tv,
        ViewHdr *__restrict__ hdr, EntryGeo *__restrict__ geo, EntryAux *__restrict__ aux, int cap,
        unsigned long long *__restrict__ stats) {
-    __shared__ int s_idx_all[kCullWarps][kCullChunk];
+    __shared__ float4 s_p0[kCullChunk], s_p1[kCullChunk];
+    __shared__ uint16_t s_idx_all[kCullWarps][kCullChunk];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int view = blockIdx.x * kCullWarps + warp;
-    if (view >= n_views) return;
-    int *s_idx = s_idx_all[warp];
+    const int wl = blockIdx.x / groups_per_world;                       // world within the rendered range
+    const int a = (blockIdx.x % groups_per_world) * kCullWarps + warp;
+    const bool active = a < sc.A;                                       // idle warps still join the barriers
+    const int view = wl * sc.A + a;
+    uint16_t *s_idx = s_idx_all[warp];
     const unsigned lt_mask = (1u << lane) - 1u;
-    const int w = world_begin + view / sc.A, a = view % sc.A;
+    const int w = world_begin + wl;
     const gp_prim *wp = prims + (size_t)w * sc.P;
-    const float2 pc = __ldg(&pitch[(size_t)w * sc.A + a]);
-    CullCam cam;
-    cam.cp = pc.x; cam.sp = pc.y;
-    // C2 camera (contract operations)
-    const float4 e0 = __ldg(reinterpret_cast<const float4 *>(&wp[a]));        // cx cy cz hx
-    const float4 e1 = __ldg(reinterpret_cast<const float4 *>(&wp[a]) + 1);    // hy hz ck sk
-    const float e_hx = e0.w, e_ck = e1.z, e_sk = e1.w;
-    cam.ox = c_fma(e_hx, e_ck, e0.x); cam.oy = c_fma(e_hx, e_sk, e0.y);
-    cam.oz = sc.cam_h;
-    cam.fx = c_mul(cam.cp, e_ck); cam.fy = c_mul(cam.cp, e_sk);
-    cam.rx = e_sk; cam.ry = -e_ck;
-    cam.ux = -c_mul(cam.sp, e_ck); cam.uy = -c_mul(cam.sp, e_sk);
+    CullCam cam = {};
+    if (active) {
+        const float2 pc = __ldg(&pitch[(size_t)w * sc.A + a]);
+        cam.cp = pc.x; cam.sp = pc.y;
+        // C2 camera (contract operations)
+        const float4 e0 = __ldg(reinterpret_cast<const float4 *>(&wp[a]));        // cx cy cz hx
+        const float4 e1 = __ldg(reinterpret_cast<const float4 *>(&wp[a]) + 1);    // hy hz ck sk
+        const float e_hx = e0.w, e_ck = e1.z, e_sk = e1.w;
+        cam.ox = c_fma(e_hx, e_ck, e0.x); cam.oy = c_fma(e_hx, e_sk, e0.y);
+        cam.oz = sc.cam_h;
+        cam.fx = c_mul(cam.cp, e_ck); cam.fy = c_mul(cam.cp, e_sk);
+        cam.rx = e_sk; cam.ry = -e_ck;
+        cam.ux = -c_mul(cam.sp, e_ck); cam.uy = -c_mul(cam.sp, e_sk);
+    }
 
     EntryGeo *vgeo = geo + (size_t)view * cap;
     EntryAux *vaux = aux + (size_t)view * cap;
@@ -121,37 +137,63 @@ k_cull(SceneConst sc, const gp_prim *__restrict__ prims, const float2 *__restric
     const float inv_th = 1.0f / th, inv_tv = 1.0f / tv;
     int cnt = 0, rmin = 0x1fff;            // list length (warp-uniform), first row touched (per lane)
 
+    // bounding-sphere pre-test constants: |n| of the side planes (-th, +-1, 0) and (-tv, 0, +-1)
+    const float sth = sqrtf(fmaf(th, th, 1.0f)) * 1.0001f, stv = sqrtf(fmaf(tv, tv, 1.0f)) * 1.0001f;
+    const float far_lim = sc.t_max * (1.0f + 1e-6f);
+    const float msc = 2.0f + th + tv;
+
     for (int k0 = 0; k0 < sc.P; k0 += kCullChunk) {
-        // ---- phase 1: one primitive per lane: frustum test, survivors compacted (ballot) into s_idx
         const int k1 = min(sc.P, k0 + kCullChunk);
+        if (k0) __syncthreads();                                         // previous round fully consumed
+        for (int i = threadIdx.x; i < k1 - k0; i += blockDim.x) {
+            const float4 *rec = reinterpret_cast<const float4 *>(&wp[k0 + i]);
+            s_p0[i] = __ldg(rec); s_p1[i] = __ldg(rec + 1);
+        }
+        __syncthreads();
+        if (!active) continue;
+        // ---- phase 1: one primitive per lane: bounding sphere against the view volume in the camera
+        // frame (looser than the exact box test of phase 2 by construction: the support of the box
+        // along any unit direction is <= R); survivors compacted (ballot) into s_idx
         int m = 0;
         for (int kb = k0; kb < k1; kb += 32) {
             const int k = kb + lane;
             bool pass = false;
             if (k < k1 && k != a) {
-                CullPrim q;
-                cull_hoist(wp, k, cam, q);
-                pass = cull_in_frustum(q, th, tv, sc.t_max);
+                const float4 p0 = s_p0[k - k0];                                           // cx cy cz hx
+                const float2 p1 = *reinterpret_cast<const float2 *>(&s_p1[k - k0]);       // hy hz
+                const float dx = p0.x - cam.ox, dy = p0.y - cam.oy, dz = p0.z - cam.oz;
+                const float R = sqrtf(fmaf(p0.w, p0.w, fmaf(p1.x, p1.x, p1.y * p1.y))) * 1.0001f;
+                const float X = fmaf(dx, cam.fx, fmaf(dy, cam.fy, dz * cam.sp));
+                const float Y = fmaf(dx, cam.rx, dy * cam.ry);
+                const float Z = fmaf(dx, cam.ux, fmaf(dy, cam.uy, dz * cam.cp));
+                const float E = fmaf(1e-5f, fabsf(dx) + fabsf(dy) + fabsf(dz) + R, 1e-6f);
+                const float mg = E * msc;
+                pass = X + R >= -E && X - R <= far_lim + E &&
+                       fabsf(Y) - th * X <= fmaf(R, sth, mg) && fabsf(Z) - tv * X <= fmaf(R, stv, mg);
             }
             const unsigned mask = __ballot_sync(0xffffffffu, pass);
-            if (pass) s_idx[m + __popc(mask & lt_mask)] = k;
+            if (pass) s_idx[m + __popc(mask & lt_mask)] = (uint16_t)(k - k0);
             m += __popc(mask);
         }
         __syncwarp();
-        // ---- phase 2: dense over the survivors: pixel bounds by corner projection, list append
+        // ---- phase 2: dense over the survivors: exact box-vs-view-volume test, then pixel bounds by
+        // corner projection (4 corners for a flat primitive, 8 for a box), list append
         for (int ib = 0; ib < m; ib += 32) {
         const int it = ib + lane;
         bool keep = false;
         EntryGeo g; EntryAux x;
-        if (it < m) {
-        const int k = s_idx[it];
         CullPrim q;
-        cull_hoist(wp, k, cam, q);
+        if (it < m) {
+            cull_hoist(s_p0[s_idx[it]], s_p1[s_idx[it]], cam, q);
+            keep = cull_in_frustum(q, th, tv, sc.t_max);
+        }
+        if (keep) {
+        const int k = k0 + s_idx[it];
         g = q.g;
         const float E = q.E, Xc = q.Xc, Yc = q.Yc, Zc = q.Zc, Xr = q.Xr;
         const float Xx = q.Xx, Xy = q.Xy, Xz = q.Xz, Yx = q.Yx, Yy = q.Yy, Zx = q.Zx, Zy = q.Zy, Zz = q.Zz;
         const float hz = q.hz;
-        keep = true;
+        const int nc = hz == 0.0f ? 4 : 8;        // flat: the corners c and c + 4 coincide
         // corner projection with near-plane clipping
         float cX[8], cY[8], cZ[8];
 #pragma unroll
@@ -166,17 +208,22 @@ k_cull(SceneConst sc, const gp_prim *__restrict__ prims, const float2 *__restric
         const float near = kNearEps;
         if (Xc - Xr >= near + E) {
 #pragma unroll
-            for (int c = 0; c < 8; ++c) bound_point(b, cX[c], cY[c], cZ[c], E);
+            for (int c = 0; c < 4; ++c) bound_point(b, cX[c], cY[c], cZ[c], E);
+            if (nc == 8) {
+#pragma unroll
+                for (int c = 4; c < 8; ++c) bound_point(b, cX[c], cY[c], cZ[c], E);
+            }
         } else if (Xc + Xr < near + E) {
             full = true;                                                  // thin sliver in front of the camera plane
         } else {
             float qYmin = 3.0e38f, qYmax = -3.0e38f, qZmin = 3.0e38f, qZmax = -3.0e38f;   // cross-section at X = near
 #pragma unroll
             for (int c = 0; c < 8; ++c) {
+                if (c >= nc) break;
                 if (cX[c] >= near) bound_point(b, cX[c], cY[c], cZ[c], E);
 #pragma unroll
                 for (int bit = 1; bit < 8; bit <<= 1) {
-                    if (c & bit) continue;
+                    if ((c & bit) || bit >= nc) continue;
                     const int d = c | bit;
                     const float Xa = cX[c], Xb = cX[d];
                     if ((Xa < near) == (Xb < near)) continue;
@@ -220,6 +267,7 @@ k_cull(SceneConst sc, const gp_prim *__restrict__ prims, const float2 *__restric
         }
         __syncwarp();
     }
+    if (!active) return;
     rmin = __reduce_min_sync(0xffffffffu, rmin);
     if (lane == 0) {
         ViewHdr h; h.n = cnt | (rmin << 19); h.oz = cam.oz; h.cp = cam.cp; h.sp = cam.sp;

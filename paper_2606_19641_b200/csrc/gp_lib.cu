@@ -286,8 +286,9 @@ static int render_device(gp_ctx *c, int world_begin, int n_worlds, int H, int W,
     if (rc != GP_OK) return rc;
     {
         LaunchTimer lt(c, GP_KERNEL_CULL, stream);
-        k_cull<<<(unsigned)((views + kCullWarps - 1) / kCullWarps), kCullWarps * 32, 0, stream>>>(
-            sc, c->d_prims, c->d_pitch, world_begin, (int)views, H, W, th, tv,
+        const int gpw = (sc.A + kCullWarps - 1) / kCullWarps;      // CTAs per world
+        k_cull<<<(unsigned)((size_t)n_worlds * gpw), kCullWarps * 32, 0, stream>>>(
+            sc, c->d_prims, c->d_pitch, world_begin, gpw, H, W, th, tv,
                                                     c->d_hdr, c->d_geo, c->d_aux, c->scratch_cap, stats);
     }
     c->launches += 1;
