@@ -115,7 +115,8 @@ int gp_cameras_set(gp_ctx *ctx, const float *d_pitch_cs, void *stream);
  *   d_instance [n][H][W]    int32   the winning primitive's inst; -1 for ground and sky
  *   d_depth    [n][H][W]    float   planar depth of the nearest hit; 0 for sky
  *   d_rgb      [n][3][H][W] uint8   shaded colour, planar; NULL skips the plane
- * 1 <= H, W <= 4096.  The fast path needs W % 4 == 0; other widths take the brute-force path.
+ * 1 <= H, W <= 4096.  The fast path needs W >= 4 and (H * W) % 4 == 0 (e.g. 210 x 126, 434 x 252);
+ * other sizes take the brute-force path.
  * May grow library-owned scratch on first use of a larger (n_worlds, H, W): warm up before timing. */
 int gp_render_batch(gp_ctx *ctx, int world_begin, int n_worlds, int agents, int H, int W,
                     float fov_rad, uint8_t *d_class, int32_t *d_instance, float *d_depth,

@@ -94,6 +94,58 @@ __device__ __forceinline__ void resolve_quad(float tg, const uint4 *s_bg, const 
     }
 }
 
+// The same for 4 consecutive pixels that straddle two image rows (W % 4 != 0): the first `nsplit`
+// pixels lie on the row with ground depth tga, the others on the next row (tgb).
+__device__ __forceinline__ void resolve_quad_split(float tga, float tgb, int nsplit, const uint4 *s_bg,
+                                                   const unsigned long long *kq, const uint32_t *__restrict__ wtab,
+                                                   uint8_t *pc, int32_t *pi, float *pd, uint8_t *pr, size_t HW) {
+    float tgv[4];
+    uint32_t m = 0;                                        // byte mask of the pixels whose background is ground
+#pragma unroll
+    for (int e = 0; e < 4; ++e) {
+        tgv[e] = e < nsplit ? tga : tgb;
+        if (tgv[e] > 0.0f) m |= 0xffu << (8 * e);
+    }
+    const uint4 sky = s_bg[0], gnd = s_bg[1];
+    uint32_t cls4 = (gnd.x & m) | (sky.x & ~m), r4 = (gnd.y & m) | (sky.y & ~m);
+    uint32_t g4 = (gnd.z & m) | (sky.z & ~m), b4 = (gnd.w & m) | (sky.w & ~m);
+    int4 inst4 = make_int4(-1, -1, -1, -1);
+    float4 dep4 = make_float4(fmaxf(tgv[0], 0.0f), fmaxf(tgv[1], 0.0f), fmaxf(tgv[2], 0.0f), fmaxf(tgv[3], 0.0f));
+    if (kq) {
+        const ulonglong2 ka = *reinterpret_cast<const ulonglong2 *>(kq);
+        const ulonglong2 kb = *reinterpret_cast<const ulonglong2 *>(kq + 2);
+        if ((ka.x & ka.y & kb.x & kb.y) != kKeyEmpty) {
+#define GP_PATCH(KEY, E, SEL, IF, DF)                                                          \
+            if ((KEY) != kKeyEmpty) {                                                          \
+                const float t = __uint_as_float((uint32_t)((KEY) >> 32));                      \
+                if (!(tgv[E] > 0.0f) || t <= tgv[E]) {     /* else the ground is nearer (C6) */ \
+                    const uint32_t lo = (uint32_t)(KEY);                                       \
+                    const uint32_t cw = __ldg(&wtab[lo]);                                      \
+                    IF = (int)__ldg(&wtab[lo | 6u]);                                           \
+                    DF = t;                                                                    \
+                    cls4 = __byte_perm(cls4, cw >> 24, SEL);                                   \
+                    r4 = __byte_perm(r4, cw, SEL);                                             \
+                    g4 = __byte_perm(g4, cw >> 8, SEL);                                        \
+                    b4 = __byte_perm(b4, cw >> 16, SEL);                                       \
+                }                                                                              \
+            }
+            GP_PATCH(ka.x, 0, 0x3214, inst4.x, dep4.x)
+            GP_PATCH(ka.y, 1, 0x3240, inst4.y, dep4.y)
+            GP_PATCH(kb.x, 2, 0x3410, inst4.z, dep4.z)
+            GP_PATCH(kb.y, 3, 0x4210, inst4.w, dep4.w)
+#undef GP_PATCH
+        }
+    }
+    *reinterpret_cast<uint32_t *>(pc) = cls4;
+    *reinterpret_cast<int4 *>(pi) = inst4;
+    *reinterpret_cast<float4 *>(pd) = dep4;
+    if (pr) {
+        *reinterpret_cast<uint32_t *>(pr) = r4;
+        *reinterpret_cast<uint32_t *>(pr + HW) = g4;
+        *reinterpret_cast<uint32_t *>(pr + 2 * HW) = b4;
+    }
+}
+
 // Contract C5 (per-pixel part) + C6 for one ray against one staged entry: exact fp32 slab test and
 // lexicographic-minimum update of the pixel's key.  g0 = (ax bx ay by), g1 = (az bz . .); dlx, dly are
 // the box-frame direction (already formed with the contract's fma chain), rt = (v, dz, 1/dz, tg).
@@ -341,10 +393,16 @@ k_render(SceneConst sc, RenderArgs ra) {
                                  pi + it * 128, pd + it * 128, pr ? pr + it * 128 : nullptr, HW);
                 }
             } else {
+                // any W: the strip is SR*W consecutive pixels (a multiple of 4, start 4-aligned); a lane's
+                // 4 pixels straddle two rows only when W % 4 != 0
                 int row = row0 + lane_row, col = lane_col, off = 0;
                 while (row <= row1) {
-                    resolve_quad(s_row[row].w, s_bg, kq ? kq + off : nullptr, wtab, pc + off, pi + off, pd + off,
-                                 pr ? pr + off : nullptr, HW);
+                    if (col + 4 <= W)
+                        resolve_quad(s_row[row].w, s_bg, kq ? kq + off : nullptr, wtab, pc + off, pi + off, pd + off,
+                                     pr ? pr + off : nullptr, HW);
+                    else
+                        resolve_quad_split(s_row[row].w, s_row[row + 1].w, W - col, s_bg, kq ? kq + off : nullptr, wtab,
+                                           pc + off, pi + off, pd + off, pr ? pr + off : nullptr, HW);
                     off += 128; row += step_row; col += step_col;
                     if (col >= W) { col -= W; ++row; }
                 }

@@ -270,7 +270,8 @@ static int render_device(gp_ctx *c, int world_begin, int n_worlds, int H, int W,
     unsigned long long *stats = c->opt_stats ? c->d_stats : nullptr;
     if (stats) CK(cudaMemsetAsync(stats, 0, 2 * sizeof(unsigned long long), stream));
 
-    if (c->opt_path == GP_PATH_BRUTE || (W & 3)) {
+    // fast path: every view (H*W pixels) must start 16-byte aligned in the 32-bit planes
+    if (c->opt_path == GP_PATH_BRUTE || W < 4 || (((long long)H * W) & 3)) {
         const int HW = H * W;
         dim3 grid((unsigned)views, (unsigned)std::min((HW + 255) / 256, 65535));
         {
@@ -301,7 +302,7 @@ static int render_device(gp_ctx *c, int world_begin, int n_worlds, int H, int W,
     // >= 16 strips to spread over its warps (a strip's entries are processed serially by one warp)
     int strip_px = c->opt_strip_px;
     if (strip_px <= 0) { strip_px = 512; while (strip_px > 128 && H * W / strip_px < 16) strip_px /= 2; }
-    int SR = 1;
+    int SR = (W & 1) ? 4 : (W & 2) ? 2 : 1;                    // strips start on a multiple of 4 pixels
     while (SR < 16 && SR * 2 * W <= strip_px) SR *= 2;
     ra.SR = SR;
     const int LR = SR < 4 ? SR : 4;
