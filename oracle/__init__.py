@@ -19,20 +19,37 @@ _PRIM_BYTES = 48
 class Params(ctypes.Structure):
     _fields_ = [("cam_height", ctypes.c_float), ("t_max", ctypes.c_float),
                 ("fov_rad", ctypes.c_float), ("ambient", ctypes.c_float),
-                ("light", ctypes.c_float * 3), ("palette", (ctypes.c_uint8 * 3) * 4)]
+                ("light", ctypes.c_float * 3), ("palette", (ctypes.c_uint8 * 3) * 8)]
+
+
+class Cam(ctypes.Structure):
+    """One camera of the per-agent rig: cos / sin of the yaw offset (positive = left), mount position
+    along the agent's axis in half lengths (+1 front-centre, -1 rear-centre)."""
+    _fields_ = [("cd", ctypes.c_float), ("sd", ctypes.c_float), ("mount", ctypes.c_float)]
+
+
+PALETTE = ((135, 206, 235), (90, 90, 90), (240, 240, 240), (40, 80, 220),
+           (220, 60, 60), (240, 160, 40), (150, 110, 70), (250, 240, 80))
 
 
 def make_params(cam_height=1.6, t_max=100.0, fov_rad=np.float32(np.pi / 2), ambient=0.25,
-                light=(0.48, 0.36, 0.8),
-                palette=((135, 206, 235), (90, 90, 90), (240, 240, 240), (40, 80, 220))) -> Params:
+                light=(0.48, 0.36, 0.8), palette=PALETTE) -> Params:
     p = Params()
     p.cam_height, p.t_max, p.fov_rad, p.ambient = cam_height, t_max, float(fov_rad), ambient
     for i in range(3):
         p.light[i] = light[i]
-    for c in range(4):
+    for c in range(8):
         for ch in range(3):
-            p.palette[c][ch] = int(palette[c][ch])
+            p.palette[c][ch] = int(palette[c][ch]) if c < len(palette) else 0
     return p
+
+
+def _cam(cam):
+    if cam is None:
+        return None
+    c = Cam()
+    c.cd, c.sd, c.mount = float(np.float32(cam[0])), float(np.float32(cam[1])), float(np.float32(cam[2]))
+    return ctypes.byref(c)
 
 
 _lib = None
@@ -43,10 +60,10 @@ def lib():
     if _lib is None:
         L = ctypes.CDLL(_build())
         vp, ci, cf = ctypes.c_void_p, ctypes.c_int, ctypes.c_float
-        L.orc_render_view.argtypes = [vp, ci, ci, cf, cf, ctypes.POINTER(Params), ci, ci,
+        L.orc_render_view.argtypes = [vp, ci, ci, cf, cf, vp, ctypes.POINTER(Params), ci, ci,
                                       vp, vp, vp, vp, vp, vp]
         L.orc_render_view.restype = ci
-        L.orc_shadow_view.argtypes = [vp, ci, ci, cf, cf, ctypes.POINTER(Params), ci, ci,
+        L.orc_shadow_view.argtypes = [vp, ci, ci, cf, cf, vp, ctypes.POINTER(Params), ci, ci,
                                       vp, vp, vp, vp]
         L.orc_shadow_view.restype = ci
         _lib = L
@@ -59,9 +76,9 @@ def _check_prims(prims):
     return prims
 
 
-def render_view(prims, ego, H, W, params=None, cp=1.0, sp=0.0, rgb=True):
+def render_view(prims, ego, H, W, params=None, cp=1.0, sp=0.0, rgb=True, cam=None):
     """fp32-contract render of one view.  prims: 1-D structured array (48-byte records) of the
-    ego's world.  Returns dict(cls u8[H,W], inst i32[H,W], depth f32[H,W], rgb u8[3,H,W] or None,
+    ego's world.  cam: (cos d, sin d, mount) of the rig camera, None = the front camera (1, 0, 1).  Returns dict(cls u8[H,W], inst i32[H,W], depth f32[H,W], rgb u8[3,H,W] or None,
     t2 f32[H,W], win i32[H,W])."""
     prims = _check_prims(prims)
     params = params or make_params()
@@ -69,7 +86,7 @@ def render_view(prims, ego, H, W, params=None, cp=1.0, sp=0.0, rgb=True):
            "depth": np.empty((H, W), np.float32),
            "rgb": np.empty((3, H, W), np.uint8) if rgb else None,
            "t2": np.empty((H, W), np.float32), "win": np.empty((H, W), np.int32)}
-    rc = lib().orc_render_view(prims.ctypes.data, len(prims), int(ego), float(cp), float(sp),
+    rc = lib().orc_render_view(prims.ctypes.data, len(prims), int(ego), float(cp), float(sp), _cam(cam),
                                ctypes.byref(params), H, W,
                                out["cls"].ctypes.data, out["inst"].ctypes.data, out["depth"].ctypes.data,
                                out["rgb"].ctypes.data if rgb else None,
@@ -79,13 +96,13 @@ def render_view(prims, ego, H, W, params=None, cp=1.0, sp=0.0, rgb=True):
     return out
 
 
-def shadow_view(prims, ego, H, W, params=None, cp=1.0, sp=0.0):
+def shadow_view(prims, ego, H, W, params=None, cp=1.0, sp=0.0, cam=None):
     """fp64 face-enumeration render of one view: dict(win i32, depth f64, t2 f64, ndl f64)."""
     prims = _check_prims(prims)
     params = params or make_params()
     out = {"win": np.empty((H, W), np.int32), "depth": np.empty((H, W), np.float64),
            "t2": np.empty((H, W), np.float64), "ndl": np.empty((H, W), np.float64)}
-    rc = lib().orc_shadow_view(prims.ctypes.data, len(prims), int(ego), float(cp), float(sp),
+    rc = lib().orc_shadow_view(prims.ctypes.data, len(prims), int(ego), float(cp), float(sp), _cam(cam),
                                ctypes.byref(params), H, W, out["win"].ctypes.data,
                                out["depth"].ctypes.data, out["t2"].ctypes.data, out["ndl"].ctypes.data)
     if rc != 0:
@@ -94,17 +111,20 @@ def shadow_view(prims, ego, H, W, params=None, cp=1.0, sp=0.0):
 
 
 def render_views(world_prims, views, H, W, params=None, pitch_cs=None, rgb=True, threads=1,
-                 shadow=False):
-    """Render a list of (world, agent) views.  world_prims: [Wn][P] structured array.  The
+                 shadow=False, rig=None):
+    """Render a list of (world, agent) or, with a rig [(cos d, sin d, mount), ...], (world, agent,
+    camera) views.  world_prims: [Wn][P] structured array.  The
     renderer itself is single-threaded; `threads` > 1 runs the same code over disjoint views
     (ctypes releases the GIL).  Returns a list of dicts in the order of `views`."""
     params = params or make_params()
 
     def one(wa):
-        w, a = wa
+        w, a = wa[0], wa[1]
         cp, sp = (1.0, 0.0) if pitch_cs is None else (float(pitch_cs[w, a, 0]), float(pitch_cs[w, a, 1]))
         fn = shadow_view if shadow else render_view
         kw = {} if shadow else {"rgb": rgb}
+        if len(wa) > 2:
+            kw["cam"] = rig[wa[2]]
         return fn(world_prims[w], a, H, W, params, cp, sp, **kw)
 
     if threads <= 1:

@@ -49,8 +49,16 @@ typedef struct {
     float fov_rad;          /* horizontal field of view                                 */
     float ambient;          /* C8                                                       */
     float light[3];         /* C8, unit vector                                          */
-    uint8_t palette[4][3];  /* sky, ground, marking, vehicle                            */
+    uint8_t palette[8][3];  /* sky, ground, marking, vehicle, + 4 user classes          */
 } orc_params;
+
+/* One camera of the per-agent rig (contract C2, NEXT-2 of SURVEY.md 8(f); "the ego
+ * camera is an entity", :319 "number of cameras configurable", :434-435 four cameras: front,
+ * front-left, front-right, rear).  cd, sd = cos / sin of the camera's yaw offset from the agent's
+ * heading (positive = to the left); mount = position along the agent's x axis in units of its half
+ * length (+1 front-centre, 0 centre, -1 rear-centre).  The default (1, 0, 1) is the single front
+ * camera of BASELINE.json configs[0]. */
+typedef struct { float cd, sd, mount; } orc_cam;
 
 /* C0: min / max that return the non-NaN operand (IEEE minNum / maxNum). */
 static float c_min(float a, float b) { if (a != a) return b; if (b != b) return a; return (b < a) ? b : a; }
@@ -70,7 +78,7 @@ static int shade_scale(float ndl, float ambient)
  * rgb[3*H*W] u8 planar (may be NULL), t2[H*W] f32 second-nearest candidate depth (+inf if
  * none; may be NULL), win[H*W] i32 winning primitive index (-1 ground, -2 sky; may be NULL).
  * Returns 0, or -1 on bad arguments. */
-int orc_render_view(const orc_prim *prims, int P, int ego, float cp, float sp,
+int orc_render_view(const orc_prim *prims, int P, int ego, float cp, float sp, const orc_cam *cam,
                     const orc_params *par, int H, int W,
                     uint8_t *cls, int32_t *inst, float *depth, uint8_t *rgb,
                     float *t2_out, int32_t *win_out)
@@ -78,13 +86,17 @@ int orc_render_view(const orc_prim *prims, int P, int ego, float cp, float sp,
     if (!prims || !par || P < 1 || ego < 0 || ego >= P || H < 1 || W < 1) return -1;
     const orc_prim *e = &prims[ego];
 
-    /* C2 camera */
-    float ox = fmaf(e->hx, e->ck, e->cx);
-    float oy = fmaf(e->hx, e->sk, e->cy);
+    /* C2 camera: mount point on the agent's axis, heading = agent yaw + camera yaw offset */
+    float cd = cam ? cam->cd : 1.0f, sd = cam ? cam->sd : 0.0f, mount = cam ? cam->mount : 1.0f;
+    float hm = e->hx * mount;
+    float ox = fmaf(hm, e->ck, e->cx);
+    float oy = fmaf(hm, e->sk, e->cy);
     float oz = par->cam_height;
-    float fx = cp * e->ck, fy = cp * e->sk, fz = sp;
-    float rx = e->sk, ry = -e->ck, rz = 0.0f;
-    float ux = -(sp * e->ck), uy = -(sp * e->sk), uz = cp;
+    float ckc = fmaf(e->ck, cd, -(e->sk * sd));
+    float skc = fmaf(e->sk, cd, e->ck * sd);
+    float fx = cp * ckc, fy = cp * skc, fz = sp;
+    float rx = skc, ry = -ckc, rz = 0.0f;
+    float ux = -(sp * ckc), uy = -(sp * skc), uz = cp;
     float th = (float)tan(0.5 * (double)par->fov_rad);
     float tv = th * ((float)H / (float)W);
     float t_max = par->t_max;
@@ -173,7 +185,7 @@ int orc_render_view(const orc_prim *prims, int P, int ego, float cp, float sp,
             if (win_out) win_out[px] = best_k;
             if (rgb) {
                 size_t plane = (size_t)H * (size_t)W;
-                int pc = (c >= 0 && c < 4) ? c : 0;
+                int pc = (c >= 0 && c < 8) ? c : 0;
                 for (int ch = 0; ch < 3; ++ch) {
                     int base = par->palette[pc][ch];
                     rgb[(size_t)ch * plane + px] = (uint8_t)((c == 0) ? base : ((base * s8) >> 8));
@@ -187,16 +199,20 @@ int orc_render_view(const orc_prim *prims, int P, int ego, float cp, float sp,
 /* fp64 shadow renderer: face enumeration in the world frame.  Outputs win[H*W] (winning
  * primitive index, -1 ground, -2 sky), depth[H*W] (0 for sky), t2[H*W] (second-nearest
  * candidate, +inf if none), ndl[H*W] (max(n.L, 0) of the entry face; 0 for sky). */
-int orc_shadow_view(const orc_prim *prims, int P, int ego, float cp_f, float sp_f,
+int orc_shadow_view(const orc_prim *prims, int P, int ego, float cp_f, float sp_f, const orc_cam *cam,
                     const orc_params *par, int H, int W,
                     int32_t *win, double *depth, double *t2_out, double *ndl_out)
 {
     if (!prims || !par || P < 1 || ego < 0 || ego >= P || H < 1 || W < 1) return -1;
     const orc_prim *e = &prims[ego];
     double cp = cp_f, sp = sp_f;
-    double eck = e->ck, esk = e->sk;
-    double o[3] = { (double)e->cx + (double)e->hx * eck, (double)e->cy + (double)e->hx * esk,
+    /* the agent's heading rotated by the camera's yaw offset (2x2 rotation applied to the unit
+     * heading vector), mount point along the agent's own axis */
+    double cd = cam ? cam->cd : 1.0, sd = cam ? cam->sd : 0.0, mount = cam ? cam->mount : 1.0;
+    double ack = e->ck, ask = e->sk;
+    double o[3] = { (double)e->cx + mount * (double)e->hx * ack, (double)e->cy + mount * (double)e->hx * ask,
                     (double)par->cam_height };
+    double eck = cd * ack - sd * ask, esk = sd * ack + cd * ask;
     double f[3] = { cp * eck, cp * esk, sp };
     double r[3] = { esk, -eck, 0.0 };
     double u[3] = { -sp * eck, -sp * esk, cp };
