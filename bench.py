@@ -113,8 +113,8 @@ def workload_cfg(args):
 
 
 def config_dict(cfg, extra=None):
-    d = {"workload": "%s: %d worlds x %d agents + %d quads, %dx%d px, %.0f m extent, 4 planes" % (
-        cfg.name, cfg.n_worlds, cfg.agents, cfg.quads, cfg.H, cfg.W, cfg.extent),
+    d = {"workload": "%s: %d worlds x %d agents x %d camera(s) + %d quads, %dx%d px (HxW), %.0f m extent, 4 planes" % (
+        cfg.name, cfg.n_worlds, cfg.agents, cfg.cams, cfg.quads, cfg.H, cfg.W, cfg.extent),
         "baseline_config": "BASELINE.json configs[2] (paper-scale)" if cfg.name == "paper" else cfg.name,
         "views_per_step": cfg.views, "pixels_per_step": cfg.views * cfg.H * cfg.W,
         "l2": "outputs per step (%.2f GB) far exceed the 126 MB L2; no explicit flush" % (cfg.views * cfg.H * cfg.W * 12 / 1e9)}
@@ -127,16 +127,18 @@ def config_dict(cfg, extra=None):
 def oracle_sample(cfg, n_views, threads):
     """The oracle as it stands over the first n_views views of the workload (frame 0); returns seconds."""
     import oracle
-    n_w = (n_views + cfg.agents - 1) // cfg.agents
+    vpw = cfg.agents * cfg.cams
+    n_w = (n_views + vpw - 1) // vpw
     sub = cfg.replace(n_worlds=n_w)
     agents, quads = gs.gen_world_prims(sub)
     prims = np.concatenate([agents, quads], axis=1)
     pitch = gs.gen_pitch(sub) if cfg.pitch_deg_max > 0 else None
     par = oracle.make_params(cam_height=cfg.cam_height, t_max=cfg.t_max, fov_rad=float(np.float32(cfg.fov_rad)))
-    views = [(v // cfg.agents, v % cfg.agents) for v in range(n_views)]
-    oracle.render_views(prims, views[:threads], cfg.H, cfg.W, par, pitch_cs=pitch, threads=threads)   # page in
+    rig = gs.rig_array(cfg.rig)
+    views = [(v // vpw, (v % vpw) // cfg.cams, v % cfg.cams) for v in range(n_views)]
+    oracle.render_views(prims, views[:threads], cfg.H, cfg.W, par, pitch_cs=pitch, threads=threads, rig=rig)   # page in
     t0 = time.perf_counter()
-    oracle.render_views(prims, views, cfg.H, cfg.W, par, pitch_cs=pitch, threads=threads)
+    oracle.render_views(prims, views, cfg.H, cfg.W, par, pitch_cs=pitch, threads=threads, rig=rig)
     return time.perf_counter() - t0
 
 
@@ -197,6 +199,8 @@ def run_b200(args):
     r.scene_upload(agents, quads, cam_height=cfg.cam_height, t_max=cfg.t_max)
     if cfg.pitch_deg_max > 0:
         r.cameras_set(torch.from_numpy(gs.gen_pitch(big, w0, cfg.n_worlds)).to(dev))
+    if cfg.rig != gs.RIG_FRONT:
+        r.camera_rig_set(gs.rig_array(cfg.rig))
     outs = r.alloc_outputs(cfg.views, cfg.H, cfg.W, rgb=True)
 
     def step(f):

@@ -14,5 +14,6 @@ from .generator import (  # noqa: F401
     PRIM_DTYPE, SceneConfig, CONFIGS, config, gen_world_prims, gen_dynamics,
     gen_pitch, poses_at_frames, splitmix64_stream, CLASS_SKY, CLASS_GROUND,
     CLASS_MARKING, CLASS_VEHICLE, DEFAULT_PALETTE, DEFAULT_LIGHT,
-    DEFAULT_AMBIENT,
+    DEFAULT_AMBIENT, CLASS_PEDESTRIAN, CLASS_CYCLIST, CLASS_OBSTACLE, CLASS_LIGHT,
+    RIG_FRONT, RIG_PAPER4, rig_array,
 )

@@ -23,8 +23,27 @@ import math
 import numpy as np
 
 CLASS_SKY, CLASS_GROUND, CLASS_MARKING, CLASS_VEHICLE = 0, 1, 2, 3
+CLASS_PEDESTRIAN, CLASS_CYCLIST, CLASS_OBSTACLE, CLASS_LIGHT = 4, 5, 6, 7      # PAPER.md:62 entity kinds
 DEFAULT_PALETTE = np.array(
-    [[135, 206, 235], [90, 90, 90], [240, 240, 240], [40, 80, 220]], dtype=np.uint8)
+    [[135, 206, 235], [90, 90, 90], [240, 240, 240], [40, 80, 220],
+     [220, 60, 60], [240, 160, 40], [150, 110, 70], [250, 240, 80]], dtype=np.uint8)
+
+# Camera rigs: (yaw offset in degrees, positive = left; mount along the agent's axis in half lengths).
+RIG_FRONT = ((0.0, 1.0),)                                         # BASELINE.json configs[0]
+RIG_PAPER4 = ((0.0, 1.0), (60.0, 1.0), (-60.0, 1.0), (180.0, -1.0))  # front, front-left, front-right, rear (PAPER.md:434)
+
+
+def rig_array(rig) -> np.ndarray:
+    """[C][4] fp32 = (cos d, sin d, mount, 0) of a rig given as ((deg, mount), ...)."""
+    out = np.zeros((len(rig), 4), dtype=np.float32)
+    for i, (deg, mount) in enumerate(rig):
+        q = round(deg / 90.0)
+        if abs(deg - 90.0 * q) < 1e-12:          # exact quarter turns
+            c, s_ = [(1.0, 0.0), (0.0, 1.0), (-1.0, 0.0), (0.0, -1.0)][q % 4]
+        else:
+            c, s_ = math.cos(math.radians(deg)), math.sin(math.radians(deg))
+        out[i] = (c, s_, mount, 0.0)
+    return out
 DEFAULT_LIGHT = (0.48, 0.36, 0.8)
 DEFAULT_AMBIENT = 0.25
 
@@ -59,14 +78,20 @@ class SceneConfig:
     cam_height: float = 1.6
     rgb: bool = True
     dt: float = 0.1
+    rig: tuple = RIG_FRONT          # cameras per agent
+    class_mix: bool = False         # some agents become vans (taller than the camera), pedestrians, cyclists
 
     @property
     def prims(self) -> int:
         return self.agents + self.quads
 
     @property
+    def cams(self) -> int:
+        return len(self.rig)
+
+    @property
     def views(self) -> int:
-        return self.n_worlds * self.agents
+        return self.n_worlds * self.agents * len(self.rig)
 
     @property
     def fov_rad(self) -> float:
@@ -83,6 +108,9 @@ CONFIGS = {
     "paper": SceneConfig("paper", 2, 1024, 64, 200, 150.0, 128, 128),
     "sweep": SceneConfig("sweep", 3, 512, 64, 200, 150.0, 128, 128),
     "dense": SceneConfig("dense", 4, 2048, 128, 500, 100.0, 256, 256, pitch_deg_max=5.0),
+    # the paper's training cameras (4 cameras at 210 x 126) and
+    # entity kinds (vehicles, pedestrians, cyclists) on the paper-scale world recipe
+    "rig4": SceneConfig("rig4", 5, 256, 64, 200, 150.0, 126, 210, rig=RIG_PAPER4, class_mix=True),
 }
 
 
@@ -162,6 +190,20 @@ def gen_world_prims(cfg: SceneConfig, world_begin: int = 0, n_worlds: int | None
         agents["cos_yaw"] = np.cos(yaw); agents["sin_yaw"] = np.sin(yaw)
         agents["cls"] = CLASS_VEHICLE
         agents["inst"] = np.arange(A, dtype=np.int32)[None, :]
+        if cfg.class_mix:
+            # kind from the length draw u = L - 4: [0,.7) car, [.7,.8) van 3.2 m tall (taller than the
+            # camera), [.8,.9) pedestrian 0.6 x 0.6 x 1.8, [.9,1) cyclist 1.8 x 0.6 x 1.7; footprints only
+            # shrink, so the overlap rejection still holds
+            u = Ls - 4.0
+            van, ped, cyc = (u >= .7) & (u < .8), (u >= .8) & (u < .9), u >= .9
+            hx, hy, hz = agents["hx"].copy(), agents["hy"].copy(), agents["hz"].copy()
+            hz[van] = 1.6
+            hx[ped] = 0.3; hy[ped] = 0.3; hz[ped] = 0.9
+            hx[cyc] = 0.9; hy[cyc] = 0.3; hz[cyc] = 0.85
+            agents["hx"] = hx; agents["hy"] = hy; agents["hz"] = hz; agents["cz"] = hz
+            cls = agents["cls"].copy()
+            cls[ped] = CLASS_PEDESTRIAN; cls[cyc] = CLASS_CYCLIST
+            agents["cls"] = cls
     quads = np.zeros((n, Q), dtype=PRIM_DTYPE)
     if Q:
         keys = _stream_keys(cfg.seed, worlds, _STREAM_QUADS)

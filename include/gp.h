@@ -17,7 +17,8 @@
  *  - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Calls enqueue
  *    work on it and return without synchronising, except where stated.
  *  - Only sm_100 (B200) devices are accepted; there is no fallback path of any kind.
- *  - Views are ordered world-major, then agent: view = world * agents_per_world + agent.
+ *  - Views are ordered world-major, then agent, then camera of the rig (gp_camera_rig_set; one front
+ *    camera by default): view = (world * agents_per_world + agent) * n_cams + cam.
  */
 #ifndef GP_H_
 #define GP_H_
@@ -70,15 +71,27 @@ typedef struct {
     float t_max;                /* far plane on planar depth, metres (100); +inf allowed      */
     float light[3];             /* unit vector towards the light (0.48, 0.36, 0.8)            */
     float ambient;              /* in [0,1] (0.25)                                            */
-    uint8_t palette[4][3];      /* RGB of class 0 sky, 1 ground, 2 marking, 3 vehicle         */
+    uint8_t palette[8][3];      /* RGB of class 0 sky, 1 ground, 2 marking, 3 vehicle, 4-7 user
+                                   classes (pedestrian, cyclist, obstacle, light: PAPER.md:62)  */
 } gp_scene_desc;
+
+#define GP_MAX_CAMS 8
+
+/* One camera of the per-agent rig (C2; PAPER.md:317 "the ego camera is an entity", :319
+ * "number of cameras configurable", :434 front / front-left / front-right / rear).  16 bytes. */
+typedef struct {
+    float cos_yaw_off, sin_yaw_off;   /* yaw offset from the agent's heading, positive = to the left   */
+    float mount;                      /* position on the agent's x axis in half lengths: +1 front-centre,
+                                         0 centre, -1 rear-centre                                      */
+    float pad;
+} gp_camera;
 
 /* One primitive: an oriented box; hz == 0 makes it a flat quad (C1).  48 bytes. */
 typedef struct {
     float cx, cy, cz;           /* centre, world frame: z up                                  */
     float hx, hy, hz;           /* half extents along the box axes, >= 0                      */
     float cos_yaw, sin_yaw;     /* heading of the box x axis                                  */
-    int32_t cls;                /* class id written to the class plane (0..3)                 */
+    int32_t cls;                /* class id written to the class plane (0..7)                 */
     int32_t inst;               /* instance id written to the instance plane                  */
     int32_t pad[2];
 } gp_prim;
@@ -108,9 +121,16 @@ int gp_agents_update(gp_ctx *ctx, const float *d_pose, void *stream);
  * NULL resets every camera to pitch 0.  Copied on `stream`. */
 int gp_cameras_set(gp_ctx *ctx, const float *d_pitch_cs, void *stream);
 
+/* The camera rig shared by all agents: h_rig HOST [n_cams], 1 <= n_cams <= GP_MAX_CAMS, copied before
+ * the call returns.  Default after gp_create: one camera (1, 0, +1) = front-centre, looking ahead.
+ * Takes effect for renders enqueued afterwards; the pitch set by gp_cameras_set applies to every
+ * camera of an agent. */
+int gp_camera_rig_set(gp_ctx *ctx, int n_cams, const gp_camera *h_rig);
+
 /* Steps a1-a9.  Renders the views of worlds [world_begin, world_begin + n_worlds) at H x W pixels with
  * horizontal field of view fov_rad (vertical follows from square pixels).  `agents` must equal
- * agents_per_world.  Outputs (DEVICE, 16-byte aligned, n = n_worlds*agents views, row-major, row 0 = top):
+ * agents_per_world.  Outputs (DEVICE, 16-byte aligned, n = n_worlds*agents*n_cams views, row-major,
+ * row 0 = top):
  *   d_class    [n][H][W]    uint8   0 sky, 1 ground, else the winning primitive's cls
  *   d_instance [n][H][W]    int32   the winning primitive's inst; -1 for ground and sky
  *   d_depth    [n][H][W]    float   planar depth of the nearest hit; 0 for sky

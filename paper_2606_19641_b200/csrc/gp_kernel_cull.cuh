@@ -98,7 +98,7 @@ __device__ __forceinline__ bool cull_in_frustum(const CullPrim &q, float th, flo
 constexpr int kCullChunk = 320;        // primitives staged in shared memory per round
 constexpr int kCullWarps = 8;          // views per CTA (one warp per view), all of the same world
 
-// Grid: one CTA per (world, group of kCullWarps agents).  The world's records (first 32 bytes of each:
+// Grid: one CTA per (world, group of kCullWarps views of that world).  The world's records (first 32 bytes of each:
 // centre, half extents, heading) are staged in shared memory once per CTA and shared by its views.
 __global__ void __launch_bounds__(kCullWarps * 32, 3)
 k_cull(SceneConst sc, const gp_prim *__restrict__ prims, const float2 *__restrict__ pitch,
@@ -109,9 +109,10 @@ k_cull(SceneConst sc, const gp_prim *__restrict__ prims, const float2 *__restric
     __shared__ uint16_t s_idx_all[kCullWarps][kCullChunk];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int wl = blockIdx.x / groups_per_world;                       // world within the rendered range
-    const int a = (blockIdx.x % groups_per_world) * kCullWarps + warp;
-    const bool active = a < sc.A;                                       // idle warps still join the barriers
-    const int view = wl * sc.A + a;
+    const int v = (blockIdx.x % groups_per_world) * kCullWarps + warp;  // view within the world
+    const bool active = v < sc.A * sc.C;                                // idle warps still join the barriers
+    const int a = v / sc.C, cam_id = v - a * sc.C;
+    const int view = wl * sc.A * sc.C + v;
     uint16_t *s_idx = s_idx_all[warp];
     const unsigned lt_mask = (1u << lane) - 1u;
     const int w = world_begin + wl;
@@ -123,8 +124,9 @@ k_cull(SceneConst sc, const gp_prim *__restrict__ prims, const float2 *__restric
         // C2 camera (contract operations)
         const float4 e0 = __ldg(reinterpret_cast<const float4 *>(&wp[a]));        // cx cy cz hx
         const float4 e1 = __ldg(reinterpret_cast<const float4 *>(&wp[a]) + 1);    // hy hz ck sk
-        const float e_hx = e0.w, e_ck = e1.z, e_sk = e1.w;
-        cam.ox = c_fma(e_hx, e_ck, e0.x); cam.oy = c_fma(e_hx, e_sk, e0.y);
+        const CamPose cq = rig_camera(sc, cam_id, e0, e1);
+        const float e_ck = cq.ck, e_sk = cq.sk;
+        cam.ox = cq.ox; cam.oy = cq.oy;
         cam.oz = sc.cam_h;
         cam.fx = c_mul(cam.cp, e_ck); cam.fy = c_mul(cam.cp, e_sk);
         cam.rx = e_sk; cam.ry = -e_ck;

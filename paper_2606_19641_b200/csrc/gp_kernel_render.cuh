@@ -233,7 +233,7 @@ k_render(SceneConst sc, RenderArgs ra) {
     }
     __syncthreads();                       // tables + mbarrier init visible
 
-    const int w = ra.world_begin + view / sc.A;
+    const int w = ra.world_begin + view / (sc.A * sc.C);
     const uint32_t *wtab = reinterpret_cast<const uint32_t *>(ra.meta + (size_t)w * sc.P);   // uint32[P][8]
     const int LC = 1 << ra.log2LC, LR = 32 >> ra.log2LC;
     const int li = lane >> ra.log2LC, lj = lane & (LC - 1);

@@ -12,7 +12,7 @@ __device__ __forceinline__ void write_meta(const gp_prim &p, PrimMeta *out, cons
     float q[3] = {qx, qy, sc.Lz};
     PrimMeta m;
     m.inst = p.inst; m.inst_dup = p.inst;
-    const uint32_t c = (uint32_t)p.cls & 3u;
+    const uint32_t c = (uint32_t)p.cls & 7u;
 #pragma unroll
     for (int a = 0; a < 3; ++a) {
         const int lo = shade_scale(c_max(-q[a], 0.0f), sc.ambient);    // sigma = -1
@@ -59,16 +59,18 @@ k_render_brute(SceneConst sc, const gp_prim *__restrict__ prims, const float2 *_
                uint8_t *__restrict__ o_cls, int32_t *__restrict__ o_inst, float *__restrict__ o_depth,
                uint8_t *__restrict__ o_rgb) {
     const int view = blockIdx.x;
-    const int w = world_begin + view / sc.A, a = view % sc.A;
+    const int va = view / sc.C, cam = view - va * sc.C;
+    const int w = world_begin + va / sc.A, a = va % sc.A;
     const gp_prim *wp = prims + (size_t)w * sc.P;
     const float2 pc = pitch[(size_t)w * sc.A + a];
     const float cp = pc.x, sp = pc.y;
     const gp_prim e = wp[a];
     // C2
-    const float ox = c_fma(e.hx, e.cos_yaw, e.cx), oy = c_fma(e.hx, e.sin_yaw, e.cy), oz = sc.cam_h;
-    const float fx = c_mul(cp, e.cos_yaw), fy = c_mul(cp, e.sin_yaw);
-    const float rx = e.sin_yaw, ry = -e.cos_yaw;
-    const float ux = -c_mul(sp, e.cos_yaw), uy = -c_mul(sp, e.sin_yaw);
+    const CamPose cq = rig_camera(sc, cam, make_float4(e.cx, e.cy, e.cz, e.hx), make_float4(e.hy, e.hz, e.cos_yaw, e.sin_yaw));
+    const float ox = cq.ox, oy = cq.oy, oz = sc.cam_h;
+    const float fx = c_mul(cp, cq.ck), fy = c_mul(cp, cq.sk);
+    const float rx = cq.sk, ry = -cq.ck;
+    const float ux = -c_mul(sp, cq.ck), uy = -c_mul(sp, cq.sk);
     const int HW = H * W;
     for (int px = blockIdx.y * blockDim.x + threadIdx.x; px < HW; px += gridDim.y * blockDim.x) {
         const int i = px / W, j = px - i * W;
@@ -130,7 +132,7 @@ k_render_brute(SceneConst sc, const gp_prim *__restrict__ prims, const float2 *_
         const size_t o = (size_t)view * HW + px;
         o_cls[o] = (uint8_t)c; o_inst[o] = id; o_depth[o] = dep;
         if (o_rgb) {
-            const uint32_t pal = sc.pal[c & 3];
+            const uint32_t pal = sc.pal[c & 7];
             const uint32_t rgb = c == 0 ? pal : shade_rgb(pal, s8);
             const size_t ob = (size_t)view * 3 * HW + px;
             o_rgb[ob] = (uint8_t)(rgb & 0xff); o_rgb[ob + HW] = (uint8_t)((rgb >> 8) & 0xff);

@@ -94,6 +94,8 @@ extern "C" int gp_create(gp_ctx **out, int cuda_device) {
     gp_ctx *c = new (std::nothrow) gp_ctx();
     if (!c) return GP_ERR_NOMEM;
     c->device = cuda_device;
+    c->sc.C = 1;                                                   // default rig: one front camera
+    c->sc.rig[0] = make_float4(1.0f, 0.0f, 1.0f, 0.0f);
     cudaError_t e = cudaMalloc(&c->d_stats, 2 * sizeof(unsigned long long));
     if (e != cudaSuccess) { delete c; return cuda_fail(e, "cudaMalloc(stats)"); }
     cudaMemset(c->d_stats, 0, 2 * sizeof(unsigned long long));
@@ -160,11 +162,11 @@ extern "C" int gp_scene_upload(gp_ctx *c, const gp_scene_desc *d, const gp_prim 
     const size_t Wn = d->n_worlds, A = d->agents_per_world, Q = d->quads_per_world, n = Wn * (size_t)P;
     for (size_t i = 0; i < Wn * A; ++i) {
         const gp_prim &p = h_agents[i];
-        if (p.cls < 0 || p.cls > 3 || !(p.hx >= 0.0f && p.hy >= 0.0f && p.hz >= 0.0f)) return GP_ERR_ARG;
+        if (p.cls < 0 || p.cls > 7 || !(p.hx >= 0.0f && p.hy >= 0.0f && p.hz >= 0.0f)) return GP_ERR_ARG;
     }
     for (size_t i = 0; i < Wn * Q; ++i) {
         const gp_prim &p = h_quads[i];
-        if (p.cls < 0 || p.cls > 3 || !(p.hx >= 0.0f && p.hy >= 0.0f && p.hz >= 0.0f)) return GP_ERR_ARG;
+        if (p.cls < 0 || p.cls > 7 || !(p.hx >= 0.0f && p.hy >= 0.0f && p.hz >= 0.0f)) return GP_ERR_ARG;
     }
     cudaStream_t stream = static_cast<cudaStream_t>(stream_);
     CK(cudaSetDevice(c->device));
@@ -190,7 +192,7 @@ extern "C" int gp_scene_upload(gp_ctx *c, const gp_scene_desc *d, const gp_prim 
     sc.Wn = (int)Wn; sc.A = (int)A; sc.Q = (int)Q; sc.P = (int)P;
     sc.cam_h = d->cam_height; sc.t_max = d->t_max;
     sc.Lx = d->light[0]; sc.Ly = d->light[1]; sc.Lz = d->light[2]; sc.ambient = d->ambient;
-    for (int k = 0; k < 4; ++k)
+    for (int k = 0; k < 8; ++k)
         sc.pal[k] = (uint32_t)d->palette[k][0] | ((uint32_t)d->palette[k][1] << 8) | ((uint32_t)d->palette[k][2] << 16);
     CK(cudaMemcpyAsync(c->d_prims, c->h_stage, n * sizeof(gp_prim), cudaMemcpyHostToDevice, stream));
     k_prim_meta<<<(unsigned)((n + 255) / 256), 256, 0, stream>>>(sc, c->d_prims, c->d_meta);
@@ -231,6 +233,18 @@ extern "C" int gp_cameras_set(gp_ctx *c, const float *d_pitch_cs, void *stream_)
     return GP_OK;
 }
 
+extern "C" int gp_camera_rig_set(gp_ctx *c, int n_cams, const gp_camera *h_rig) {
+    if (!c || !h_rig || n_cams < 1 || n_cams > GP_MAX_CAMS) return GP_ERR_ARG;
+    for (int i = 0; i < n_cams; ++i) {
+        const gp_camera &q = h_rig[i];
+        if (!(fabsf(q.cos_yaw_off) <= 1.0f && fabsf(q.sin_yaw_off) <= 1.0f && fabsf(q.mount) <= 16.0f)) return GP_ERR_ARG;
+    }
+    c->sc.C = n_cams;
+    for (int i = 0; i < n_cams; ++i)
+        c->sc.rig[i] = make_float4(h_rig[i].cos_yaw_off, h_rig[i].sin_yaw_off, h_rig[i].mount, 0.0f);
+    return GP_OK;
+}
+
 static int ensure_scratch(gp_ctx *c, size_t views) {
     const int cap = c->sc.P;
     if (c->scratch_views >= views && c->scratch_cap == cap) return GP_OK;
@@ -265,7 +279,7 @@ static int render_device(gp_ctx *c, int world_begin, int n_worlds, int H, int W,
     const SceneConst &sc = c->sc;
     const float th = (float)tan(0.5 * (double)fov_rad);          // C2, host side
     const float tv = th * ((float)H / (float)W);
-    const size_t views = (size_t)n_worlds * sc.A;
+    const size_t views = (size_t)n_worlds * sc.A * sc.C;
     if (views > 0x7fffffffull) return GP_ERR_ARG;
     unsigned long long *stats = c->opt_stats ? c->d_stats : nullptr;
     if (stats) CK(cudaMemsetAsync(stats, 0, 2 * sizeof(unsigned long long), stream));
@@ -287,7 +301,7 @@ static int render_device(gp_ctx *c, int world_begin, int n_worlds, int H, int W,
     if (rc != GP_OK) return rc;
     {
         LaunchTimer lt(c, GP_KERNEL_CULL, stream);
-        const int gpw = (sc.A + kCullWarps - 1) / kCullWarps;      // CTAs per world
+        const int gpw = (sc.A * sc.C + kCullWarps - 1) / kCullWarps;   // CTAs per world
         k_cull<<<(unsigned)((size_t)n_worlds * gpw), kCullWarps * 32, 0, stream>>>(
             sc, c->d_prims, c->d_pitch, world_begin, gpw, H, W, th, tv,
                                                     c->d_hdr, c->d_geo, c->d_aux, c->scratch_cap, stats);
@@ -361,7 +375,7 @@ extern "C" int gp_render_batch_host(gp_ctx *c, const float *h_pose, int world_be
     if (!h_class || !h_instance || !h_depth) return GP_ERR_ARG;
     cudaStream_t stream = static_cast<cudaStream_t>(stream_);
     const SceneConst &sc = c->sc;
-    const size_t HW = (size_t)H * W, A = sc.A;
+    const size_t HW = (size_t)H * W, A = (size_t)sc.A * sc.C;      // A: views per world here
     const size_t bpv = HW * (h_rgb ? 12 : 9);                     // output bytes per view
     // chunk: <= 512 MiB of planes per staging buffer, at least one world
     size_t wc = (512ull << 20) / (bpv * A);
@@ -385,7 +399,7 @@ extern "C" int gp_render_batch_host(gp_ctx *c, const float *h_pose, int world_be
         c->d_out_bytes = need;
     }
     if (h_pose) {
-        CK(cudaMemcpyAsync(c->d_pose, h_pose, (size_t)sc.Wn * A * 4 * sizeof(float), cudaMemcpyHostToDevice, stream));
+        CK(cudaMemcpyAsync(c->d_pose, h_pose, (size_t)sc.Wn * sc.A * 4 * sizeof(float), cudaMemcpyHostToDevice, stream));
         rc = gp_agents_update(c, c->d_pose, stream);
         if (rc != GP_OK) return rc;
     }

@@ -21,7 +21,7 @@ GP_PATH_FAST, GP_PATH_BRUTE = 0, 1
 
 EXPORTS = ("gp_create", "gp_destroy", "gp_set_option", "gp_scene_upload", "gp_agents_update",
            "gp_cameras_set", "gp_render_batch", "gp_render_batch_host", "gp_stats", "gp_kernel_time",
-           "gp_launch_count",
+           "gp_launch_count", "gp_camera_rig_set",
            "gp_error_string")
 
 
@@ -29,7 +29,16 @@ class SceneDesc(ctypes.Structure):
     _fields_ = [("n_worlds", ctypes.c_int32), ("agents_per_world", ctypes.c_int32),
                 ("quads_per_world", ctypes.c_int32), ("cam_height", ctypes.c_float),
                 ("t_max", ctypes.c_float), ("light", ctypes.c_float * 3), ("ambient", ctypes.c_float),
-                ("palette", (ctypes.c_uint8 * 3) * 4)]
+                ("palette", (ctypes.c_uint8 * 3) * 8)]
+
+
+class Camera(ctypes.Structure):
+    _fields_ = [("cos_yaw_off", ctypes.c_float), ("sin_yaw_off", ctypes.c_float), ("mount", ctypes.c_float),
+                ("pad", ctypes.c_float)]
+
+
+DEFAULT_PALETTE = ((135, 206, 235), (90, 90, 90), (240, 240, 240), (40, 80, 220),
+                   (220, 60, 60), (240, 160, 40), (150, 110, 70), (250, 240, 80))
 
 
 class GpError(RuntimeError):
@@ -61,6 +70,7 @@ def lib():
         L.gp_stats.argtypes = [vp, ctypes.POINTER(ctypes.c_uint64), ctypes.POINTER(ctypes.c_uint64)]
         L.gp_kernel_time.argtypes = [vp, ci, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_uint64)]
         L.gp_launch_count.argtypes = [vp, ctypes.POINTER(ctypes.c_uint64)]
+        L.gp_camera_rig_set.argtypes = [vp, ci, vp]
         L.gp_error_string.argtypes = [ci]
         L.gp_error_string.restype = ctypes.c_char_p
         for name in EXPORTS[:-1]:
@@ -91,6 +101,7 @@ class Renderer:
         _check(lib().gp_create(ctypes.byref(self._h), int(device)))
         self.device = int(device)
         self.desc = None
+        self.n_cams = 1
 
     def close(self):
         if getattr(self, "_h", None):
@@ -103,8 +114,7 @@ class Renderer:
         _check(lib().gp_set_option(self._h, key, value))
 
     def scene_upload(self, agents: np.ndarray, quads: np.ndarray | None, cam_height=1.6, t_max=100.0,
-                     light=(0.48, 0.36, 0.8), ambient=0.25,
-                     palette=((135, 206, 235), (90, 90, 90), (240, 240, 240), (40, 80, 220))):
+                     light=(0.48, 0.36, 0.8), ambient=0.25, palette=DEFAULT_PALETTE):
         """agents [Wn][A], quads [Wn][Q] (or None): host arrays of 48-byte gp_prim records."""
         agents = np.ascontiguousarray(agents)
         assert agents.ndim == 2 and agents.dtype.itemsize == 48
@@ -119,7 +129,7 @@ class Renderer:
         d.cam_height, d.t_max, d.ambient = cam_height, t_max, ambient
         for i in range(3):
             d.light[i] = light[i]
-        for c in range(4):
+        for c in range(min(8, len(palette))):
             for ch in range(3):
                 d.palette[c][ch] = int(palette[c][ch])
         _check(lib().gp_scene_upload(self._h, ctypes.byref(d), agents.ctypes.data,
@@ -134,8 +144,18 @@ class Renderer:
         """d_pitch_cs: CUDA float32 tensor [Wn][A][2] = (cos p, sin p), or None for pitch 0."""
         _check(lib().gp_cameras_set(self._h, _dptr(d_pitch_cs), _stream()))
 
+    def camera_rig_set(self, rig):
+        """rig: array-like [C][>=3] = (cos yaw offset, sin yaw offset, mount) per camera of every agent."""
+        rig = np.asarray(rig, dtype=np.float32)
+        arr = (Camera * len(rig))()
+        for i, r in enumerate(rig):
+            arr[i].cos_yaw_off, arr[i].sin_yaw_off, arr[i].mount, arr[i].pad = float(r[0]), float(r[1]), float(r[2]), 0.0
+        _check(lib().gp_camera_rig_set(self._h, len(rig), ctypes.cast(arr, ctypes.c_void_p)))
+        self.n_cams = len(rig)
+
     def render_batch(self, world_begin, n_worlds, H, W, fov_rad, d_class, d_instance, d_depth, d_rgb=None):
-        """Outputs: CUDA tensors uint8 [n][H][W], int32 [n][H][W], float32 [n][H][W], uint8 [n][3][H][W]."""
+        """Outputs: CUDA tensors uint8 [n][H][W], int32 [n][H][W], float32 [n][H][W], uint8 [n][3][H][W],
+        n = n_worlds * agents * cameras."""
         _check(lib().gp_render_batch(self._h, int(world_begin), int(n_worlds), int(self.desc.agents_per_world),
                                      int(H), int(W), float(fov_rad), _dptr(d_class), _dptr(d_instance),
                                      _dptr(d_depth), _dptr(d_rgb), _stream()))

@@ -27,7 +27,7 @@ def gpu_render(renderer, cfg, world_begin, n_worlds, path=0, rgb=True, H=None, W
     from paper_2606_19641_b200 import gp
     H = H or cfg.H; W = W or cfg.W
     renderer.set_option(gp.GP_OPT_PATH, path)
-    outs = renderer.alloc_outputs(n_worlds * cfg.agents, H, W, rgb=rgb)
+    outs = renderer.alloc_outputs(n_worlds * cfg.agents * renderer.n_cams, H, W, rgb=rgb)
     for t in outs:
         if t is not None:
             t.fill_(0x5A if t.dtype == torch.uint8 else 123456)      # poison: every element must be written
@@ -69,9 +69,10 @@ def compare_views(gpu_planes, view_indices, refs):
     return rep
 
 
-def oracle_refs(prims, views, H, W, par, pitch=None, rgb=True):
+def oracle_refs(prims, views, H, W, par, pitch=None, rgb=True, rig=None):
+    """views: (world, agent) or, with rig = [C][>=3] (cos d, sin d, mount), (world, agent, camera)."""
     import oracle
-    return oracle.render_views(prims, views, H, W, par, pitch_cs=pitch, rgb=rgb, threads=oracle_threads())
+    return oracle.render_views(prims, views, H, W, par, pitch_cs=pitch, rgb=rgb, threads=oracle_threads(), rig=rig)
 
 
 def planes_equal(a, b):

@@ -47,7 +47,10 @@ def test_error_strings(libgp):
 def test_struct_layouts_match_header():
     from paper_2606_19641_b200 import gp
     import gp_scenes as gs
-    assert ctypes.sizeof(gp.SceneDesc) == 3 * 4 + 2 * 4 + 3 * 4 + 4 + 12
+    assert ctypes.sizeof(gp.SceneDesc) == 3 * 4 + 2 * 4 + 3 * 4 + 4 + 24      # palette[8][3]
+    assert ctypes.sizeof(gp.Camera) == 16
+    import oracle
+    assert tuple(map(tuple, gs.DEFAULT_PALETTE.tolist())) == tuple(gp.DEFAULT_PALETTE) == tuple(oracle.PALETTE)
     assert gs.PRIM_DTYPE.itemsize == 48
 
 
@@ -57,6 +60,7 @@ def test_null_arguments_are_rejected_without_a_gpu(libgp):
     assert libgp.gp_destroy(None) == gp.GP_ERR_ARG
     assert libgp.gp_render_batch(None, 0, 1, 1, 8, 8, 1.0, None, None, None, None, None) == gp.GP_ERR_ARG
     assert libgp.gp_stats(None, None, None) == gp.GP_ERR_ARG
+    assert libgp.gp_camera_rig_set(None, 1, None) == gp.GP_ERR_ARG
 
 
 def test_no_cpu_fallback_create_fails_loudly_without_b200(libgp):
