@@ -52,13 +52,14 @@ PRIM_DTYPE = np.dtype([
     ("cx", "<f4"), ("cy", "<f4"), ("cz", "<f4"),
     ("hx", "<f4"), ("hy", "<f4"), ("hz", "<f4"),
     ("cos_yaw", "<f4"), ("sin_yaw", "<f4"),
-    ("cls", "<i4"), ("inst", "<i4"), ("pad", "<i4", (2,)),
+    ("cls", "<i4"), ("inst", "<i4"), ("shape", "<i4"), ("pad", "<i4"),
 ])
 assert PRIM_DTYPE.itemsize == 48
 
 _GOLDEN = np.uint64(0x9E3779B97F4A7C15)
 _M1 = np.uint64(0xBF58476D1CE4E5B9)
 _M2 = np.uint64(0x94D049BB133111EB)
+SHAPE_BOX, SHAPE_SPHERE = 0, 1     # cuboids / planes (flat boxes), spheres for traffic lights
 _STREAM_VEHICLES, _STREAM_QUADS, _STREAM_DYNAMICS, _STREAM_PITCH = 0, 1, 2, 3
 
 

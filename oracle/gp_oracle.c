@@ -40,7 +40,7 @@ typedef struct {
     float hx, hy, hz;       /* half extents along the box's own axes, >= 0              */
     float ck, sk;           /* cos / sin of yaw                                         */
     int32_t cls, inst;      /* class id (2 marking, 3 vehicle), user instance id        */
-    int32_t pad0, pad1;
+    int32_t shape, pad1;    /* 0 oriented box (flat quad if hz == 0), 1 sphere of radius hx */
 } orc_prim;                 /* 48 bytes, the generator's PRIM_DTYPE                      */
 
 typedef struct {
@@ -123,6 +123,28 @@ int orc_render_view(const orc_prim *prims, int P, int ego, float cp, float sp, c
             for (int k = 0; k < P; ++k) {
                 if (k == ego) continue;
                 const orc_prim *p = &prims[k];
+                if (p->shape == 1) {
+/* C5s sphere ("traffic lights use spheres"), un-normalised world-frame
+                     * direction d, e = o - c.  Foot of the centre on the ray, then the half chord: the
+                     * well-conditioned form (no b^2 - ac cancellation). */
+                    float dx = fmaf(v, ux, fmaf(s, rx, fx));
+                    float dy = fmaf(v, uy, fmaf(s, ry, fy));
+                    float ex = ox - p->cx, ey = oy - p->cy, ez = oz - p->cz;
+                    float A = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+                    float B = fmaf(dz, ez, fmaf(dy, ey, dx * ex));
+                    float invA = 1.0f / A;
+                    float tca = (-B) * invA;
+                    float lx = fmaf(tca, dx, ex), ly = fmaf(tca, dy, ey), lz = fmaf(tca, dz, ez);
+                    float l2 = fmaf(lz, lz, fmaf(ly, ly, lx * lx));
+                    float h2 = p->hx * p->hx - l2;
+                    if (!(h2 >= 0.0f)) continue;
+                    float tn = tca - sqrtf(h2 * invA);
+                    if (!(tn > 0.0f && tn <= t_max)) continue;
+                    int wins = (tn < best_t) || (tn == best_t && best_k < 0);
+                    if (wins) { second_t = best_t; best_t = tn; best_k = k; best_m = 3; best_sigma = 1.0f; }
+                    else if (tn < second_t) second_t = tn;
+                    continue;
+                }
                 float ck = p->ck, sk = p->sk;
                 float ex = ox - p->cx, ey = oy - p->cy;
                 float olx = fmaf(sk, ey, ck * ex);
@@ -179,6 +201,7 @@ int orc_render_view(const orc_prim *prims, int P, int ego, float cp, float sp, c
                 float qz = Lz;
                 float qm = (best_m == 0) ? qx : (best_m == 1) ? qy : qz;
                 s8 = shade_scale(c_max(best_sigma * qm, 0.0f), par->ambient);
+                if (best_m == 3) s8 = 256;      /* C8: spheres (lights) are emissive, palette colour unshaded */
             }
             cls[px] = (uint8_t)c; inst[px] = id; depth[px] = dep;
             if (t2_out) t2_out[px] = second_t;
@@ -239,6 +262,21 @@ int orc_shadow_view(const orc_prim *prims, int P, int ego, float cp_f, float sp_
             for (int k = 0; k < P; ++k) {
                 if (k == ego) continue;
                 const orc_prim *p = &prims[k];
+                if (p->shape == 1) {
+/* quadratic |e + t d|^2 = r^2 solved directly (fp64 affords the cancellation) */
+                    double e3[3] = { o[0] - p->cx, o[1] - p->cy, o[2] - p->cz };
+                    double qa = d[0] * d[0] + d[1] * d[1] + d[2] * d[2];
+                    double qb = e3[0] * d[0] + e3[1] * d[1] + e3[2] * d[2];
+                    double qc = e3[0] * e3[0] + e3[1] * e3[1] + e3[2] * e3[2] - (double)p->hx * (double)p->hx;
+                    double disc = qb * qb - qa * qc;
+                    if (disc < 0.0) continue;
+                    double ts = (-qb - sqrt(disc)) / qa;
+                    if (!(ts > 0.0 && ts <= t_max)) continue;
+                    int winss = (ts < best_t) || (ts == best_t && best_k < 0);
+                    if (winss) { second_t = best_t; best_t = ts; best_k = k; best_ndl = 1.0; }
+                    else if (ts < second_t) second_t = ts;
+                    continue;
+                }
                 double c[3] = { p->cx, p->cy, p->cz };
                 double h[3] = { p->hx, p->hy, p->hz };
                 double ax[3][3] = { { p->ck, p->sk, 0.0 }, { -(double)p->sk, p->ck, 0.0 }, { 0.0, 0.0, 1.0 } };

@@ -16,13 +16,17 @@ def pytest_configure(config):
 import gp_scenes as gs  # noqa: E402
 
 
-def make_prim(cx, cy, cz, hx, hy, hz, cos_yaw=1.0, sin_yaw=0.0, cls=3, inst=0):
+def make_prim(cx, cy, cz, hx, hy, hz, cos_yaw=1.0, sin_yaw=0.0, cls=3, inst=0, shape=0):
     p = np.zeros((), dtype=gs.PRIM_DTYPE)
     p["cx"], p["cy"], p["cz"] = cx, cy, cz
     p["hx"], p["hy"], p["hz"] = hx, hy, hz
     p["cos_yaw"], p["sin_yaw"] = cos_yaw, sin_yaw
-    p["cls"], p["inst"] = cls, inst
+    p["cls"], p["inst"], p["shape"] = cls, inst, shape
     return p
+
+
+def make_sphere(cx, cy, cz, r, cls=7, inst=0):
+    return make_prim(cx, cy, cz, r, r, r, 1.0, 0.0, cls=cls, inst=inst, shape=gs.SHAPE_SPHERE)
 
 
 def ego_at_origin(cos_yaw=1.0, sin_yaw=0.0, half_len=2.0):
