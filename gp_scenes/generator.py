@@ -81,10 +81,15 @@ class SceneConfig:
     dt: float = 0.1
     rig: tuple = RIG_FRONT          # cameras per agent
     class_mix: bool = False         # some agents become vans (taller than the camera), pedestrians, cyclists
+    lights: int = 0                 # traffic-light spheres per world, appended to the static primitives
+
+    @property
+    def statics(self) -> int:
+        return self.quads + self.lights
 
     @property
     def prims(self) -> int:
-        return self.agents + self.quads
+        return self.agents + self.quads + self.lights
 
     @property
     def cams(self) -> int:
@@ -111,7 +116,7 @@ CONFIGS = {
     "dense": SceneConfig("dense", 4, 2048, 128, 500, 100.0, 256, 256, pitch_deg_max=5.0),
     # the paper's training cameras (4 cameras at 210 x 126) and
     # entity kinds (vehicles, pedestrians, cyclists) on the paper-scale world recipe
-    "rig4": SceneConfig("rig4", 5, 256, 64, 200, 150.0, 126, 210, rig=RIG_PAPER4, class_mix=True),
+    "rig4": SceneConfig("rig4", 5, 256, 64, 200, 150.0, 126, 210, rig=RIG_PAPER4, class_mix=True, lights=16),
 }
 
 
@@ -179,7 +184,7 @@ def _gen_vehicles(cfg: SceneConfig, worlds: np.ndarray):
 
 
 def gen_world_prims(cfg: SceneConfig, world_begin: int = 0, n_worlds: int | None = None):
-    """Return (agents[Wn][A], quads[Wn][Q]) structured arrays of PRIM_DTYPE at t=0."""
+    """Return (agents[Wn][A], statics[Wn][Q + lights]) structured arrays of PRIM_DTYPE at t=0."""
     n = cfg.n_worlds - world_begin if n_worlds is None else n_worlds
     worlds = np.arange(world_begin, world_begin + n)
     A, Q, E = cfg.agents, cfg.quads, cfg.extent
@@ -220,6 +225,24 @@ def gen_world_prims(cfg: SceneConfig, world_begin: int = 0, n_worlds: int | None
         quads["cos_yaw"] = np.cos(psi); quads["sin_yaw"] = np.sin(psi)
         quads["cls"] = CLASS_MARKING
         quads["inst"] = (A + np.arange(Q, dtype=np.int32))[None, :]
+    Lt = cfg.lights
+    if Lt:
+        # traffic lights: spheres of radius 0.2 m, 4-6 m up, uniform over the world;
+        # draws continue the quad stream (counters Q*4 ..)
+        keys = _stream_keys(cfg.seed, worlds, _STREAM_QUADS)
+        kk = np.repeat(keys, Lt * 4).reshape(n, Lt, 4)
+        cc = np.broadcast_to(Q * 4 + np.arange(Lt * 4).reshape(1, Lt, 4), (n, Lt, 4))
+        u = _draws(kk.ravel(), cc.ravel()).reshape(n, Lt, 4)
+        lights = np.zeros((n, Lt), dtype=PRIM_DTYPE)
+        lights["cx"] = -0.5 * E + E * u[..., 0]
+        lights["cy"] = -0.5 * E + E * u[..., 1]
+        lights["cz"] = 4.0 + 2.0 * u[..., 2]
+        lights["hx"] = 0.2; lights["hy"] = 0.2; lights["hz"] = 0.2
+        lights["cos_yaw"] = 1.0
+        lights["cls"] = CLASS_LIGHT
+        lights["shape"] = SHAPE_SPHERE
+        lights["inst"] = (A + Q + np.arange(Lt, dtype=np.int32))[None, :]
+        quads = np.concatenate([quads, lights], axis=1)
     return agents, quads
 
 

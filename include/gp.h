@@ -86,14 +86,20 @@ typedef struct {
     float pad;
 } gp_camera;
 
-/* One primitive: an oriented box; hz == 0 makes it a flat quad (C1).  48 bytes. */
+enum { GP_SHAPE_BOX = 0, GP_SHAPE_SPHERE = 1 };
+
+/* One primitive (C1; "vehicles and static objects use cuboids, road segments use
+ * planes, and traffic lights use spheres").  GP_SHAPE_BOX: an oriented box; hz == 0 makes it a flat quad.
+ * GP_SHAPE_SPHERE: a sphere of radius hx about the centre (hy, hz and the heading are ignored), drawn
+ * unshaded in its class colour (lights are emissive, C8).  48 bytes. */
 typedef struct {
     float cx, cy, cz;           /* centre, world frame: z up                                  */
     float hx, hy, hz;           /* half extents along the box axes, >= 0                      */
     float cos_yaw, sin_yaw;     /* heading of the box x axis                                  */
     int32_t cls;                /* class id written to the class plane (0..7)                 */
     int32_t inst;               /* instance id written to the instance plane                  */
-    int32_t pad[2];
+    int32_t shape;              /* GP_SHAPE_BOX or GP_SHAPE_SPHERE                            */
+    int32_t pad;
 } gp_prim;
 
 /* Create a context on CUDA device `cuda_device`.  GP_ERR_ARCH unless it is sm_100. */

@@ -106,6 +106,7 @@ k_cull(SceneConst sc, const gp_prim *__restrict__ prims, const float2 *__restric
        ViewHdr *__restrict__ hdr, EntryGeo *__restrict__ geo, EntryAux *__restrict__ aux, int cap,
        unsigned long long *__restrict__ stats) {
     __shared__ float4 s_p0[kCullChunk], s_p1[kCullChunk];
+    __shared__ uint8_t s_sphere[kCullChunk];
     __shared__ uint16_t s_idx_all[kCullWarps][kCullChunk];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int wl = blockIdx.x / groups_per_world;                       // world within the rendered range
@@ -149,7 +150,10 @@ k_cull(SceneConst sc, const gp_prim *__restrict__ prims, const float2 *__restric
         if (k0) __syncthreads();                                         // previous round fully consumed
         for (int i = threadIdx.x; i < k1 - k0; i += blockDim.x) {
             const float4 *rec = reinterpret_cast<const float4 *>(&wp[k0 + i]);
-            s_p0[i] = __ldg(rec); s_p1[i] = __ldg(rec + 1);
+            float4 p0 = __ldg(rec), p1 = __ldg(rec + 1);
+            const bool sphere = __float_as_int(__ldg(rec + 2).z) == GP_SHAPE_SPHERE;     // cls inst shape pad
+            if (sphere) { p1.x = p0.w; p1.y = p0.w; p1.z = 1.0f; p1.w = 0.0f; }          // bounding cube, heading 0
+            s_p0[i] = p0; s_p1[i] = p1; s_sphere[i] = sphere;
         }
         __syncthreads();
         if (!active) continue;
@@ -191,7 +195,11 @@ k_cull(SceneConst sc, const gp_prim *__restrict__ prims, const float2 *__restric
         }
         if (keep) {
         const int k = k0 + s_idx[it];
+        const bool sphere = s_sphere[s_idx[it]];
         g = q.g;
+        if (sphere) {       // C5s entry: e = o - c (ol with heading 0, exact) and r*r; basis slots already world-frame
+            g.ax = q.olx; g.bx = q.oly; g.ay = q.olz; g.by = c_mul(q.hx, q.hx);
+        }
         const float E = q.E, Xc = q.Xc, Yc = q.Yc, Zc = q.Zc, Xr = q.Xr;
         const float Xx = q.Xx, Xy = q.Xy, Xz = q.Xz, Yx = q.Yx, Yy = q.Yy, Zx = q.Zx, Zy = q.Zy, Zz = q.Zz;
         const float hz = q.hz;
@@ -254,7 +262,7 @@ k_cull(SceneConst sc, const gp_prim *__restrict__ prims, const float2 *__restric
             if (c0 > c1 || r0 > r1) keep = false;                         // touches no pixel centre
         }
         if (keep) rmin = min(rmin, r0);
-        x.kf = ((uint32_t)k << 1) | (hz == 0.0f ? 1u : 0u);
+        x.kf = ((uint32_t)k << 2) | (sphere ? kKindSphere : hz == 0.0f ? kKindFlat : kKindBox);
         x.rows = (uint32_t)r0 | ((uint32_t)r1 << 16);
         x.cols = (uint32_t)c0 | ((uint32_t)c1 << 16);
         x.pad = 0;

@@ -290,8 +290,9 @@ k_render(SceneConst sc, RenderArgs ra) {
                     g0 = __ldg(gg); g1 = __ldg(gg + 1); g2 = __ldg(gg + 2);
                     ax = __ldg(reinterpret_cast<const uint4 *>(&g_aux[eb]));
                 }
-                const bool flat = ax.x & 1u;
-                const uint32_t klow = (ax.x >> 1) << 3;
+                const uint32_t kind = ax.x & 3u;
+                const bool flat = kind == kKindFlat;
+                const uint32_t klow = (ax.x >> 2) << 3;
                 const int r0 = max((int)(ax.y & 0xffff), row0), r1 = min((int)(ax.y >> 16), row1);
                 const int c0 = (int)(ax.z & 0xffff), c1 = (int)(ax.z >> 16);
                 // conservative pre-test data (not contract arithmetic): box centre / half extents in
@@ -299,7 +300,28 @@ k_render(SceneConst sc, RenderArgs ra) {
                 const float mx = 0.5f * (g0.x + g0.y), my = 0.5f * (g0.z + g0.w), mz = 0.5f * (g1.x + g1.y);   // -ol
                 const float ex_ = 0.5f * (g0.y - g0.x), ey_ = 0.5f * (g0.w - g0.z), ez_ = 0.5f * (g1.y - g1.x); // h
                 const float kSlack = 2e-5f, kGrow = 1.00002f;
-                if (flat && c1 - c0 >= LC) {
+                if (kind == kKindSphere) {
+                    // C5s over the entry's pixel rectangle; g0 = (e.x, e.y, e.z, r*r), basis = world frame
+                    for (int rb = r0; rb <= r1; rb += LR) {
+                        const int i = rb + li;
+                        for (int cb = c0; cb <= c1; cb += LC) {
+                            const int j = cb + lj;
+                            if (i <= r1 && j <= c1) {
+                                if (STATS) ++n_tests;
+                                const float s = s_col[j];
+                                const float4 rt = s_row[i];
+                                const float dx = c_fma(rt.x, g2.z, c_fma(s, g2.x, g1.z));
+                                const float dy = c_fma(rt.x, g2.w, c_fma(s, g2.y, g1.w));
+                                const float tn = sphere_entry(g0.x, g0.y, g0.z, g0.w, dx, dy, rt.y);
+                                if (tn > 0.0f && tn <= t_max) {
+                                    const unsigned long long key = ((unsigned long long)__float_as_uint(tn) << 32) | klow | 5u;
+                                    unsigned long long *kp = &keys[(i - row0) * W + j];
+                                    if (key < *kp) *kp = key;
+                                }
+                            }
+                        }
+                    }
+                } else if (flat && c1 - c0 >= LC) {
                     // Wide flat primitive: per row, the plane depth t is fixed, so the footprint is one
                     // column interval.  Bound it conservatively (plain fp32 + slack) and run the exact
                     // test only inside it: a thin diagonal marking costs ~its length, not its bbox area.

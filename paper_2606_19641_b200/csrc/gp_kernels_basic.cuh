@@ -17,8 +17,9 @@ __device__ __forceinline__ void write_meta(const gp_prim &p, PrimMeta *out, cons
     for (int a = 0; a < 3; ++a) {
         const int lo = shade_scale(c_max(-q[a], 0.0f), sc.ambient);    // sigma = -1
         const int hi = shade_scale(c_max(q[a], 0.0f), sc.ambient);     // sigma = +1
-        m.face[a * 2 + 0] = (c == 0 ? sc.pal[0] : shade_rgb(sc.pal[c], lo)) | (c << 24);
-        m.face[a * 2 + 1] = (c == 0 ? sc.pal[0] : shade_rgb(sc.pal[c], hi)) | (c << 24);
+        const bool plain = c == 0 || p.shape == GP_SHAPE_SPHERE;       // sky colour / emissive sphere: unshaded
+        m.face[a * 2 + 0] = (plain ? sc.pal[c] : shade_rgb(sc.pal[c], lo)) | (c << 24);
+        m.face[a * 2 + 1] = (plain ? sc.pal[c] : shade_rgb(sc.pal[c], hi)) | (c << 24);
     }
     *out = m;
 }
@@ -86,6 +87,13 @@ k_render_brute(SceneConst sc, const gp_prim *__restrict__ prims, const float2 *_
         for (int k = 0; k < sc.P; ++k) {
             if (k == a) continue;
             const gp_prim p = wp[k];
+            if (p.shape == GP_SHAPE_SPHERE) {                       // C5s
+                const float dx = c_fma(v, ux, c_fma(s, rx, fx)), dy = c_fma(v, uy, c_fma(s, ry, fy));
+                const float tn = sphere_entry(c_sub(ox, p.cx), c_sub(oy, p.cy), c_sub(oz, p.cz), c_mul(p.hx, p.hx), dx, dy, dz);
+                if (!(tn > 0.0f && tn <= sc.t_max)) continue;
+                if (tn < best_t || (tn == best_t && best_k < 0)) { best_t = tn; best_k = k; best_m = 3; best_sigma = 1.0f; }
+                continue;
+            }
             const float ck = p.cos_yaw, sk = p.sin_yaw;
             const float ex = c_sub(ox, p.cx), ey = c_sub(oy, p.cy);
             const float olx = c_fma(sk, ey, c_mul(ck, ex));
@@ -128,6 +136,7 @@ k_render_brute(SceneConst sc, const gp_prim *__restrict__ prims, const float2 *_
             const float qy = c_fma(p.cos_yaw, sc.Ly, -c_mul(p.sin_yaw, sc.Lx));
             const float qm = best_m == 0 ? qx : best_m == 1 ? qy : sc.Lz;
             s8 = shade_scale(c_max(c_mul(best_sigma, qm), 0.0f), sc.ambient);
+            if (best_m == 3) s8 = 256;                              // C8: spheres are emissive
         }
         const size_t o = (size_t)view * HW + px;
         o_cls[o] = (uint8_t)c; o_inst[o] = id; o_depth[o] = dep;

@@ -162,11 +162,13 @@ extern "C" int gp_scene_upload(gp_ctx *c, const gp_scene_desc *d, const gp_prim 
     const size_t Wn = d->n_worlds, A = d->agents_per_world, Q = d->quads_per_world, n = Wn * (size_t)P;
     for (size_t i = 0; i < Wn * A; ++i) {
         const gp_prim &p = h_agents[i];
-        if (p.cls < 0 || p.cls > 7 || !(p.hx >= 0.0f && p.hy >= 0.0f && p.hz >= 0.0f)) return GP_ERR_ARG;
+        if (p.cls < 0 || p.cls > 7 || (p.shape != GP_SHAPE_BOX && p.shape != GP_SHAPE_SPHERE) ||
+            !(p.hx >= 0.0f && p.hy >= 0.0f && p.hz >= 0.0f)) return GP_ERR_ARG;
     }
     for (size_t i = 0; i < Wn * Q; ++i) {
         const gp_prim &p = h_quads[i];
-        if (p.cls < 0 || p.cls > 7 || !(p.hx >= 0.0f && p.hy >= 0.0f && p.hz >= 0.0f)) return GP_ERR_ARG;
+        if (p.cls < 0 || p.cls > 7 || (p.shape != GP_SHAPE_BOX && p.shape != GP_SHAPE_SPHERE) ||
+            !(p.hx >= 0.0f && p.hy >= 0.0f && p.hz >= 0.0f)) return GP_ERR_ARG;
     }
     cudaStream_t stream = static_cast<cudaStream_t>(stream_);
     CK(cudaSetDevice(c->device));
