@@ -179,7 +179,9 @@ __device__ __forceinline__ void slab_select(const float4 &g0, const float4 &g1, 
 #ifndef GP_RENDER_MIN_CTAS
 #define GP_RENDER_MIN_CTAS (32 / GP_RENDER_WARPS)
 #endif
-template <bool STATS, int NG>     // NG: 128-pixel groups per strip when W is a power of two (1, 2, 4), else 0
+// NG: 128-pixel groups per strip when W is a power of two (1, 2, 4), else 0.  SPH: the scene holds spheres
+// (scenes without any run the variant compiled without the C5s branch: it costs the strip loop registers).
+template <bool STATS, int NG, bool SPH>
 __global__ void __launch_bounds__(GP_RENDER_WARPS * 32, GP_RENDER_MIN_CTAS)
 k_render(SceneConst sc, RenderArgs ra) {
     extern __shared__ __align__(16) unsigned char smem[];
@@ -300,7 +302,7 @@ k_render(SceneConst sc, RenderArgs ra) {
                 const float mx = 0.5f * (g0.x + g0.y), my = 0.5f * (g0.z + g0.w), mz = 0.5f * (g1.x + g1.y);   // -ol
                 const float ex_ = 0.5f * (g0.y - g0.x), ey_ = 0.5f * (g0.w - g0.z), ez_ = 0.5f * (g1.y - g1.x); // h
                 const float kSlack = 2e-5f, kGrow = 1.00002f;
-                if (kind == kKindSphere) {
+                if (SPH && kind == kKindSphere) {
                     // C5s over the entry's pixel rectangle; g0 = (e.x, e.y, e.z, r*r), basis = world frame
                     for (int rb = r0; rb <= r1; rb += LR) {
                         const int i = rb + li;

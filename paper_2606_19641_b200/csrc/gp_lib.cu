@@ -19,7 +19,7 @@ using namespace gp;
 
 struct gp_ctx {
     int device = -1;
-    bool have_scene = false;
+    bool have_scene = false, has_spheres = false;
     SceneConst sc{};
     gp_prim *d_prims = nullptr;
     PrimMeta *d_meta = nullptr;
@@ -170,6 +170,9 @@ extern "C" int gp_scene_upload(gp_ctx *c, const gp_scene_desc *d, const gp_prim 
         if (p.cls < 0 || p.cls > 7 || (p.shape != GP_SHAPE_BOX && p.shape != GP_SHAPE_SPHERE) ||
             !(p.hx >= 0.0f && p.hy >= 0.0f && p.hz >= 0.0f)) return GP_ERR_ARG;
     }
+    bool spheres = false;
+    for (size_t i = 0; i < Wn * A; ++i) spheres |= h_agents[i].shape == GP_SHAPE_SPHERE;
+    for (size_t i = 0; i < Wn * Q; ++i) spheres |= h_quads[i].shape == GP_SHAPE_SPHERE;
     cudaStream_t stream = static_cast<cudaStream_t>(stream_);
     CK(cudaSetDevice(c->device));
     CK(cudaDeviceSynchronize());            // earlier work may still read the old scene
@@ -202,6 +205,7 @@ extern "C" int gp_scene_upload(gp_ctx *c, const gp_scene_desc *d, const gp_prim 
     c->launches += 2;
     CK(cudaGetLastError());
     c->have_scene = true;
+    c->has_spheres = spheres;
     return GP_OK;
 }
 
@@ -334,24 +338,23 @@ static int render_device(gp_ctx *c, int world_begin, int n_worlds, int H, int W,
     const size_t smem = 48 + (size_t)ra.scap * 64 + (size_t)H * 16 + (size_t)((W + 3) & ~3) * 4 +
                         (size_t)nwarps * SR * W * 8;
     if (smem > 227 * 1024) return GP_ERR_ARG;
+    typedef void (*RenderFn)(SceneConst, RenderArgs);
+    static const RenderFn fns[2][2][4] = {      // [spheres][stats][ng index]
+        {{k_render<false, 0, false>, k_render<false, 1, false>, k_render<false, 2, false>, k_render<false, 4, false>},
+         {k_render<true, 0, false>, k_render<true, 1, false>, k_render<true, 2, false>, k_render<true, 4, false>}},
+        {{k_render<false, 0, true>, k_render<false, 1, true>, k_render<false, 2, true>, k_render<false, 4, true>},
+         {k_render<true, 0, true>, k_render<true, 1, true>, k_render<true, 2, true>, k_render<true, 4, true>}}};
     if (smem > c->render_smem_set) {
-        CK(cudaFuncSetAttribute(k_render<false, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        CK(cudaFuncSetAttribute(k_render<false, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        CK(cudaFuncSetAttribute(k_render<false, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        CK(cudaFuncSetAttribute(k_render<false, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        CK(cudaFuncSetAttribute(k_render<true, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        CK(cudaFuncSetAttribute(k_render<true, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        CK(cudaFuncSetAttribute(k_render<true, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        CK(cudaFuncSetAttribute(k_render<true, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        for (int f = 0; f < 2; ++f)
+            for (int st = 0; st < 2; ++st)
+                for (int g = 0; g < 4; ++g)
+                    CK(cudaFuncSetAttribute(fns[f][st][g], cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         c->render_smem_set = smem;
     }
     {
         LaunchTimer lt(c, GP_KERNEL_RENDER, stream);
-        const dim3 g((unsigned)views), b(nwarps * 32);
-#define GP_LAUNCH_RENDER(ST, N) k_render<ST, N><<<g, b, smem, stream>>>(sc, ra)
-        if (stats) { if (ng == 4) GP_LAUNCH_RENDER(true, 4); else if (ng == 2) GP_LAUNCH_RENDER(true, 2); else if (ng == 1) GP_LAUNCH_RENDER(true, 1); else GP_LAUNCH_RENDER(true, 0); }
-        else { if (ng == 4) GP_LAUNCH_RENDER(false, 4); else if (ng == 2) GP_LAUNCH_RENDER(false, 2); else if (ng == 1) GP_LAUNCH_RENDER(false, 1); else GP_LAUNCH_RENDER(false, 0); }
-#undef GP_LAUNCH_RENDER
+        const RenderFn fn = fns[c->has_spheres ? 1 : 0][stats ? 1 : 0][ng == 4 ? 3 : ng];
+        fn<<<dim3((unsigned)views), dim3(nwarps * 32), smem, stream>>>(sc, ra);
     }
     c->launches += 1;
     CK(cudaGetLastError());
