@@ -41,6 +41,8 @@ def parse():
     ap.add_argument("--workload", default="paper", choices=list(gs.CONFIGS))
     ap.add_argument("--worlds", type=int, default=0, help="override the number of worlds (debug)")
     ap.add_argument("--res", type=int, default=0, help="override H = W (resolution sweep)")
+    ap.add_argument("--strip-px", type=int, default=0, help="GP_OPT_STRIP_PX override (0 = library default)")
+    ap.add_argument("--stage-cap", type=int, default=0, help="GP_OPT_STAGE_CAP override (0 = library default)")
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -196,6 +198,10 @@ def run_b200(args):
     fov = float(np.float32(cfg.fov_rad))
 
     r = Renderer(local_rank)
+    if args.strip_px:
+        r.set_option(gp.GP_OPT_STRIP_PX, args.strip_px)
+    if args.stage_cap:
+        r.set_option(gp.GP_OPT_STAGE_CAP, args.stage_cap)
     r.scene_upload(agents, quads, cam_height=cfg.cam_height, t_max=cfg.t_max)
     if cfg.pitch_deg_max > 0:
         r.cameras_set(torch.from_numpy(gs.gen_pitch(big, w0, cfg.n_worlds)).to(dev))

@@ -47,6 +47,10 @@ __device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t by
 
 constexpr unsigned long long kKeyEmpty = 0xFFFFFFFFFFFFFFFFull;
 
+// 1/x to ~1 ulp in one MUFU instruction, for the conservative (non-contract) column-interval bound of flat
+// primitives only; its error is far inside the 1e-5 relative + 0.02 px slack of that bound
+__device__ __forceinline__ float flat_rcp(float x) { float r; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+
 // a5/a7/a8/a9 for the 4 consecutive pixels a lane owns in one 128-pixel group: ground / sky default
 // from the row's t_ground, patched where a primitive's key won, then one 4-byte store per 8-bit
 // plane and one 16-byte store per 32-bit plane.
@@ -147,19 +151,21 @@ __device__ __forceinline__ void resolve_quad_split(float tga, float tgb, int nsp
 }
 
 // Contract C5 (per-pixel part) + C6 for one ray against one staged entry: exact fp32 slab test and
-// lexicographic-minimum update of the pixel's key.  g0 = (ax bx ay by), g1 = (az bz . .); dlx, dly are
-// the box-frame direction (already formed with the contract's fma chain), rt = (v, dz, 1/dz, tg).
-__device__ __forceinline__ void slab_select(const float4 &g0, const float4 &g1, float dlx, float dly,
-                                            const float4 &rt, float t_max, bool flat, uint32_t klow,
-                                            unsigned long long *kp) {
+// lexicographic-minimum update of the pixel's key.  g0 = (ax bx ay by); dlx, dly are the box-frame direction
+// (already formed with the contract's fma chain); (loz, hiz) is the z slab interval, which depends on the row
+// only and is formed once per row by slab_z; dz is the row's d.z.
+__device__ __forceinline__ void slab_z(const float4 &g1, const float4 &rt, float &loz, float &hiz) {
+    const float ta = c_mul(g1.x, rt.z), tb = c_mul(g1.y, rt.z);
+    loz = c_min(ta, tb); hiz = c_max(ta, tb);
+}
+__device__ __forceinline__ void slab_select(const float4 &g0, float dlx, float dly, float loz, float hiz, float dz,
+                                            float t_max, bool flat, uint32_t klow, unsigned long long *kp) {
     const float ix = c_rcp(dlx), iy = c_rcp(dly);
     float ta, tb;
     ta = c_mul(g0.x, ix); tb = c_mul(g0.y, ix);
     const float lox = c_min(ta, tb), hix = c_max(ta, tb);
     ta = c_mul(g0.z, iy); tb = c_mul(g0.w, iy);
     const float loy = c_min(ta, tb), hiy = c_max(ta, tb);
-    ta = c_mul(g1.x, rt.z); tb = c_mul(g1.y, rt.z);
-    const float loz = c_min(ta, tb), hiz = c_max(ta, tb);
     const float tn = c_max(c_max(lox, loy), loz);
     const float tf = c_min(c_min(hix, hiy), hiz);
     if (tn <= tf && tn > 0.0f && tn <= t_max) {
@@ -167,7 +173,7 @@ __device__ __forceinline__ void slab_select(const float4 &g0, const float4 &g1, 
         if (flat) face = 5;
         else if (lox == tn) face = 0 + (dlx > 0.0f ? 0 : 1);
         else if (loy == tn) face = 2 + (dly > 0.0f ? 0 : 1);
-        else face = 4 + (rt.y > 0.0f ? 0 : 1);
+        else face = 4 + (dz > 0.0f ? 0 : 1);
         const unsigned long long key = ((unsigned long long)__float_as_uint(tn) << 32) | klow | face;   // C6
         if (key < *kp) *kp = key;
     }
@@ -297,11 +303,6 @@ k_render(SceneConst sc, RenderArgs ra) {
                 const uint32_t klow = (ax.x >> 2) << 3;
                 const int r0 = max((int)(ax.y & 0xffff), row0), r1 = min((int)(ax.y >> 16), row1);
                 const int c0 = (int)(ax.z & 0xffff), c1 = (int)(ax.z >> 16);
-                // conservative pre-test data (not contract arithmetic): box centre / half extents in
-                // the ray-origin frame, recovered from a = -h - ol, b = h - ol
-                const float mx = 0.5f * (g0.x + g0.y), my = 0.5f * (g0.z + g0.w), mz = 0.5f * (g1.x + g1.y);   // -ol
-                const float ex_ = 0.5f * (g0.y - g0.x), ey_ = 0.5f * (g0.w - g0.z), ez_ = 0.5f * (g1.y - g1.x); // h
-                const float kSlack = 2e-5f, kGrow = 1.00002f;
                 if (SPH && kind == kKindSphere) {
                     // C5s over the entry's pixel rectangle; g0 = (e.x, e.y, e.z, r*r), basis = world frame
                     for (int rb = r0; rb <= r1; rb += LR) {
@@ -327,6 +328,10 @@ k_render(SceneConst sc, RenderArgs ra) {
                     // Wide flat primitive: per row, the plane depth t is fixed, so the footprint is one
                     // column interval.  Bound it conservatively (plain fp32 + slack) and run the exact
                     // test only inside it: a thin diagonal marking costs ~its length, not its bbox area.
+                    // (not contract arithmetic: centre -ol and half extents h in the ray-origin frame, recovered from
+                    // a = -h - ol, b = h - ol)
+                    const float mx = 0.5f * (g0.x + g0.y), my = 0.5f * (g0.z + g0.w), mz = 0.5f * (g1.x + g1.y);
+                    const float ex_ = 0.5f * (g0.y - g0.x), ey_ = 0.5f * (g0.w - g0.z);
                     const float dl_ = 2e-5f * (fabsf(mx) + fabsf(my) + fabsf(mz) + ex_ + ey_) + 1e-6f;
                     const float hxs = ex_ + dl_, hys = ey_ + dl_;
                     const float col_scale = 0.5f * (float)W / ra.th;
@@ -343,11 +348,11 @@ k_render(SceneConst sc, RenderArgs ra) {
                                 float slo = -3.0e38f, shi = 3.0e38f;
                                 bool ok = true;
                                 if (fabsf(X1) > 1e-12f) {
-                                    const float r = 1.0f / X1, a = (-hxs - X0) * r, b = (hxs - X0) * r;
+                                    const float r = flat_rcp(X1), a = (-hxs - X0) * r, b = (hxs - X0) * r;
                                     slo = fmaxf(slo, fminf(a, b)); shi = fminf(shi, fmaxf(a, b));
                                 } else ok = fabsf(X0) <= hxs;
                                 if (fabsf(Y1) > 1e-12f) {
-                                    const float r = 1.0f / Y1, a = (-hys - Y0) * r, b = (hys - Y0) * r;
+                                    const float r = flat_rcp(Y1), a = (-hys - Y0) * r, b = (hys - Y0) * r;
                                     slo = fmaxf(slo, fminf(a, b)); shi = fminf(shi, fmaxf(a, b));
                                 } else ok = ok && fabsf(Y0) <= hys;
                                 if (ok && slo <= shi) {
@@ -359,41 +364,35 @@ k_render(SceneConst sc, RenderArgs ra) {
                                 }
                             }
                         }
+                        float loz, hiz;
+                        slab_z(g1, rt, loz, hiz);
+                        unsigned long long *krow = keys + (i - row0) * W;
                         for (int j = ja + lj; __any_sync(0xffffffffu, j <= jb); j += LC) {
                             if (j <= jb) {
                                 if (STATS) ++n_tests;
                                 const float s = s_col[j];
                                 const float dlx = c_fma(rt.x, g2.z, c_fma(s, g2.x, g1.z));
                                 const float dly = c_fma(rt.x, g2.w, c_fma(s, g2.y, g1.w));
-                                slab_select(g0, g1, dlx, dly, rt, t_max, true, klow, &keys[(i - row0) * W + j]);
+                                slab_select(g0, dlx, dly, loz, hiz, rt.y, t_max, true, klow, krow + j);
                             }
                         }
                     }
                 } else {
                     for (int rb = r0; rb <= r1; rb += LR) {
-                        const int i = rb + li;
+                        const int i = min(rb + li, r1);                         // lanes past r1 idle (j loop below)
+                        const bool row_ok = rb + li <= r1;
+                        const float4 rt = s_row[i];                             // v, dz, 1/dz, tg
+                        float loz, hiz;
+                        slab_z(g1, rt, loz, hiz);                               // per row, not per pixel
+                        unsigned long long *krow = keys + (i - row0) * W;
                         for (int cb = c0; cb <= c1; cb += LC) {
                             const int j = cb + lj;
-                            if (i <= r1 && j <= c1) {
+                            if (row_ok && j <= c1) {
                                 if (STATS) ++n_tests;
                                 const float s = s_col[j];
-                                const float4 rt = s_row[i];                     // v, dz, 1/dz, tg
-                                // C5, per-pixel part
                                 const float dlx = c_fma(rt.x, g2.z, c_fma(s, g2.x, g1.z));
                                 const float dly = c_fma(rt.x, g2.w, c_fma(s, g2.y, g1.w));
-                                const float dlz = rt.y;
-                                // a3 early-out per ray: separating-axis test of the LINE o + t d against the
-                                // box (axes d x e_m).  Division-free; the slack keeps it conservative, so a
-                                // ray it rejects can never pass the exact slab test.
-                                const float adx = fabsf(dlx), ady = fabsf(dly), adz = fabsf(dlz);
-                                const float px_ = my * dlz, qx_ = mz * dly;
-                                const float py_ = mz * dlx, qy_ = mx * dlz;
-                                const float pz_ = mx * dly, qz_ = my * dlx;
-                                const bool sep =
-                                    fabsf(px_ - qx_) > fmaf(ey_, adz, ez_ * ady) * kGrow + kSlack * (fabsf(px_) + fabsf(qx_)) + 1e-12f ||
-                                    fabsf(py_ - qy_) > fmaf(ez_, adx, ex_ * adz) * kGrow + kSlack * (fabsf(py_) + fabsf(qy_)) + 1e-12f ||
-                                    fabsf(pz_ - qz_) > fmaf(ex_, ady, ey_ * adx) * kGrow + kSlack * (fabsf(pz_) + fabsf(qz_)) + 1e-12f;
-                                if (!sep) slab_select(g0, g1, dlx, dly, rt, t_max, flat, klow, &keys[(i - row0) * W + j]);
+                                slab_select(g0, dlx, dly, loz, hiz, rt.y, t_max, flat, klow, krow + j);
                             }
                         }
                     }
