@@ -322,10 +322,22 @@ static int render_device(gp_ctx *c, int world_begin, int n_worlds, int H, int W,
     // >= 16 strips to spread over its warps (a strip's entries are processed serially by one warp)
     int strip_px = c->opt_strip_px;
     if (strip_px <= 0) { strip_px = 512; while (strip_px > 128 && H * W / strip_px < 16) strip_px /= 2; }
-    int SR = (W & 1) ? 4 : (W & 2) ? 2 : 1;                    // strips start on a multiple of 4 pixels
+    const int align = (W & 1) ? 4 : (W & 2) ? 2 : 1;           // strips start on a multiple of 4 pixels
+    int SR = align;
     while (SR < 16 && SR * 2 * W <= strip_px) SR *= 2;
+    if ((W & (W - 1)) && c->opt_strip_px <= 0) {
+        // width not a power of two: a strip is resolved in groups of 128 consecutive pixels, so prefer the
+        // strip height (multiple of `align`, up to ~1024 pixels, >= 8 strips per view) whose last group is fullest
+        double best = -1.0;
+        for (int cand = align; cand <= 16; cand += align) {
+            const int px = cand * W;
+            if (cand > align && (px > 1024 || (H + cand - 1) / cand < 8)) break;
+            const double eff = (double)px / (double)(((px + 127) / 128) * 128);
+            if (eff > best + 0.02) { best = eff; SR = cand; }
+        }
+    }
     ra.SR = SR;
-    const int LR = SR < 4 ? SR : 4;
+    const int LR = SR >= 4 ? 4 : SR >= 2 ? 2 : 1;              // rows of the test tile (power of two)
     ra.log2LC = LR == 4 ? 3 : LR == 2 ? 4 : 5;
     ra.o_cls = d_class; ra.o_inst = d_instance; ra.o_depth = d_depth; ra.o_rgb = d_rgb; ra.stats = stats;
     int log2W = 0;
