@@ -107,6 +107,7 @@ k_cull(SceneConst sc, const gp_prim *__restrict__ prims, const float2 *__restric
        unsigned long long *__restrict__ stats) {
     __shared__ float4 s_p0[kCullChunk], s_p1[kCullChunk];
     __shared__ uint8_t s_sphere[kCullChunk];
+    __shared__ float s_R[kCullChunk];
     __shared__ uint16_t s_idx_all[kCullWarps][kCullChunk];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int wl = blockIdx.x / groups_per_world;                       // world within the rendered range
@@ -154,6 +155,7 @@ k_cull(SceneConst sc, const gp_prim *__restrict__ prims, const float2 *__restric
             const bool sphere = __float_as_int(__ldg(rec + 2).z) == GP_SHAPE_SPHERE;     // cls inst shape pad
             if (sphere) { p1.x = p0.w; p1.y = p0.w; p1.z = 1.0f; p1.w = 0.0f; }          // bounding cube, heading 0
             s_p0[i] = p0; s_p1[i] = p1; s_sphere[i] = sphere;
+            s_R[i] = sqrtf(fmaf(p0.w, p0.w, fmaf(p1.x, p1.x, p1.y * p1.y))) * 1.0001f;      // bounding-sphere radius
         }
         __syncthreads();
         if (!active) continue;
@@ -166,9 +168,8 @@ k_cull(SceneConst sc, const gp_prim *__restrict__ prims, const float2 *__restric
             bool pass = false;
             if (k < k1 && k != a) {
                 const float4 p0 = s_p0[k - k0];                                           // cx cy cz hx
-                const float2 p1 = *reinterpret_cast<const float2 *>(&s_p1[k - k0]);       // hy hz
                 const float dx = p0.x - cam.ox, dy = p0.y - cam.oy, dz = p0.z - cam.oz;
-                const float R = sqrtf(fmaf(p0.w, p0.w, fmaf(p1.x, p1.x, p1.y * p1.y))) * 1.0001f;
+                const float R = s_R[k - k0];
                 const float X = fmaf(dx, cam.fx, fmaf(dy, cam.fy, dz * cam.sp));
                 const float Y = fmaf(dx, cam.rx, dy * cam.ry);
                 const float Z = fmaf(dx, cam.ux, fmaf(dy, cam.uy, dz * cam.cp));
