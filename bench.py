@@ -43,6 +43,8 @@ def parse():
     ap.add_argument("--res", type=int, default=0, help="override H = W (resolution sweep)")
     ap.add_argument("--strip-px", type=int, default=0, help="GP_OPT_STRIP_PX override (0 = library default)")
     ap.add_argument("--stage-cap", type=int, default=0, help="GP_OPT_STAGE_CAP override (0 = library default)")
+    ap.add_argument("--chunk-worlds", type=int, default=0,
+                    help="worlds per gp_render_batch call (0 = as many as keep the planes under 40 GB)")
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -119,6 +121,7 @@ def config_dict(cfg, extra=None):
         cfg.name, cfg.n_worlds, cfg.agents, cfg.cams, cfg.quads, cfg.H, cfg.W, cfg.extent),
         "baseline_config": "BASELINE.json configs[2] (paper-scale)" if cfg.name == "paper" else cfg.name,
         "views_per_step": cfg.views, "pixels_per_step": cfg.views * cfg.H * cfg.W,
+        "worlds_per_render_call": (extra or {}).get("worlds_per_render_call", cfg.n_worlds),
         "l2": "outputs per step (%.2f GB) far exceed the 126 MB L2; no explicit flush" % (cfg.views * cfg.H * cfg.W * 12 / 1e9)}
     if extra:
         d.update(extra)
@@ -207,11 +210,22 @@ def run_b200(args):
         r.cameras_set(torch.from_numpy(gs.gen_pitch(big, w0, cfg.n_worlds)).to(dev))
     if cfg.rig != gs.RIG_FRONT:
         r.camera_rig_set(gs.rig_array(cfg.rig))
-    outs = r.alloc_outputs(cfg.views, cfg.H, cfg.W, rgb=True)
+    # worlds per render call: the whole batch when its planes fit (paper scale: 12.9 GB), else world chunks into a
+    # reused buffer (dense: 206 GB of planes in all)
+    vpw = cfg.agents * cfg.cams
+    chunk = args.chunk_worlds or max(1, int(40e9 // (vpw * cfg.H * cfg.W * 12)))
+    chunk = min(chunk, cfg.n_worlds)
+    chunks = [(w, min(chunk, cfg.n_worlds - w)) for w in range(0, cfg.n_worlds, chunk)]
+    outs = r.alloc_outputs(chunk * vpw, cfg.H, cfg.W, rgb=True)
+    subs = {nw: [o[:nw * vpw] for o in outs] for _, nw in chunks}
 
-    def step(f):
+    def step(f, stats_acc=None):
         r.agents_update(d_pose[f])
-        r.render_batch(0, cfg.n_worlds, cfg.H, cfg.W, fov, *outs)
+        for w_begin, nw in chunks:
+            r.render_batch(w_begin, nw, cfg.H, cfg.W, fov, *subs[nw])
+            if stats_acc is not None:
+                for k, v in r.stats().items():
+                    stats_acc[k] = stats_acc.get(k, 0) + v
 
     def barrier():
         if distributed:
@@ -245,15 +259,16 @@ def run_b200(args):
 
     # one instrumented frame (not timed): executed tests and listed pairs for the FP32 roof
     r.set_option(gp.GP_OPT_STATS, 1)
-    step(n_frames - 1)
-    stats = r.stats()
+    stats = {}
+    step(n_frames - 1, stats)
     r.set_option(gp.GP_OPT_STATS, 0)
 
     # end to end through the host-buffer entry point (pinned host memory, copies inside the timed region)
     e2e = None
     if not args.no_e2e:
         try:
-            V, H, W = cfg.views, cfg.H, cfg.W
+            e2e_worlds = chunk                      # host planes of one render call (all worlds when they fit)
+            V, H, W = e2e_worlds * vpw, cfg.H, cfg.W
             h = [torch.empty((V, H, W), dtype=torch.uint8), torch.empty((V, H, W), dtype=torch.int32),
                  torch.empty((V, H, W), dtype=torch.float32), torch.empty((V, 3, H, W), dtype=torch.uint8)]
             pinned = True
@@ -263,15 +278,15 @@ def run_b200(args):
                 pinned = False
             h_pose = [torch.from_numpy(poses[f]).pin_memory() if pinned else torch.from_numpy(poses[f])
                       for f in range(min(n_frames, args.e2e_steps + 1))]
-            r.render_batch_host(h_pose[0], 0, cfg.n_worlds, H, W, fov, *h)            # warm-up, allocates staging
+            r.render_batch_host(h_pose[0], 0, e2e_worlds, H, W, fov, *h)            # warm-up, allocates staging
             barrier()
             t0 = time.perf_counter()
             for i in range(args.e2e_steps):
-                r.render_batch_host(h_pose[(i + 1) % len(h_pose)], 0, cfg.n_worlds, H, W, fov, *h)   # synchronises
+                r.render_batch_host(h_pose[(i + 1) % len(h_pose)], 0, e2e_worlds, H, W, fov, *h)   # synchronises
             barrier()
             e_s = time.perf_counter() - t0
             e_s = shard.max_over_ranks(e_s, dev)
-            e2e = {"value": world_size * cfg.views * args.e2e_steps / e_s, "unit": UNIT,
+            e2e = {"value": world_size * V * args.e2e_steps / e_s, "unit": UNIT, "worlds_per_call": e2e_worlds,
                    "h2d_bytes_per_step": int(h_pose[0].numel() * 4),
                    "d2h_bytes_per_step": int(sum(x.numel() * x.element_size() for x in h)),
                    "steps": args.e2e_steps, "pinned_host": pinned,
@@ -292,7 +307,8 @@ def run_b200(args):
     alg_bytes = npx * 12 + cfg.n_worlds * cfg.prims * 48 + cfg.views * 64
     r_ms, r_n = ktimes["render"]
     r_avg_ms = r_ms / max(1, r_n)
-    achieved = alg_bytes / (r_avg_ms * 1e-3) / 1e9
+    alg_bytes_launch = alg_bytes / len(chunks)                 # one k_render launch = one world chunk
+    achieved = alg_bytes_launch / (r_avg_ms * 1e-3) / 1e9
     traffic = None
     tpath = os.path.join(ROOT, "profiles", "r01_traffic.txt")      # from the committed ncu --set full capture
     if os.path.exists(tpath) and not args.worlds and not args.res:
@@ -309,15 +325,15 @@ def run_b200(args):
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world_size, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": step_ms, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-        "config": config_dict(cfg),
+        "config": config_dict(cfg, {"worlds_per_render_call": chunk}),
         "mpixels_per_s": value * cfg.H * cfg.W / 1e6,
         "clocks": clocks,
         "gpu_launches": int(launches),
-        "kernels_ms_per_step": {k: v[0] / max(1, v[1]) for k, v in ktimes.items()},
+        "kernels_ms_per_step": {k: v[0] / max(1, args.steps) for k, v in ktimes.items()},
         "roofline": {"bound": "hbm", "kernel": "k_render", "achieved": achieved, "peak": peak, "unit": "GB/s",
                      "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
-                     "algorithmic_bytes_per_launch": alg_bytes, "avg_launch_ms": r_avg_ms,
-                     "share_of_step": r_avg_ms / step_ms},
+                     "algorithmic_bytes_per_launch": alg_bytes_launch, "avg_launch_ms": r_avg_ms,
+                     "launches_per_step": len(chunks), "share_of_step": r_avg_ms * len(chunks) / step_ms},
         "roofline_step": {"t_hbm_ms": t_hbm_ms, "t_fp32_ms": t_fp32_ms, "frac_of_slower_roof": max(t_hbm_ms, t_fp32_ms) / step_ms,
                           "executed_tests": stats["executed_tests"], "listed_pairs": stats["listed_pairs"],
                           "tests_per_pixel": stats["executed_tests"] / npx, "fp32_peak_tflops": fp32_peak / 1e12,
