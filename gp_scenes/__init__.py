@@ -15,5 +15,5 @@ from .generator import (  # noqa: F401
     gen_pitch, poses_at_frames, splitmix64_stream, CLASS_SKY, CLASS_GROUND,
     CLASS_MARKING, CLASS_VEHICLE, DEFAULT_PALETTE, DEFAULT_LIGHT,
     DEFAULT_AMBIENT, CLASS_PEDESTRIAN, CLASS_CYCLIST, CLASS_OBSTACLE, CLASS_LIGHT,
-    RIG_FRONT, RIG_PAPER4, rig_array, SHAPE_BOX, SHAPE_SPHERE,
+    RIG_FRONT, RIG_PAPER4, rig_array, SHAPE_BOX, SHAPE_SPHERE, gen_lane_polylines,
 )

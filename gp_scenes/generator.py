@@ -246,6 +246,28 @@ def gen_world_prims(cfg: SceneConfig, world_begin: int = 0, n_worlds: int | None
     return agents, quads
 
 
+def gen_lane_polylines(cfg: SceneConfig, n_lines: int, pts_per_line: int = 9, step: float = 5.0,
+                       world_begin: int = 0, n_worlds: int | None = None) -> np.ndarray:
+    """Lane-like polylines [Wn][n_lines][pts_per_line][2] fp32: arcs of constant curvature ~U[-0.03, 0.03] 1/m from
+    a uniform start point and heading, vertices `step` metres apart (draws: the quad stream, counters 2^20 ..)."""
+    n = cfg.n_worlds - world_begin if n_worlds is None else n_worlds
+    worlds = np.arange(world_begin, world_begin + n)
+    E = cfg.extent
+    keys = _stream_keys(cfg.seed, worlds, _STREAM_QUADS)
+    kk = np.repeat(keys, n_lines * 4).reshape(n, n_lines, 4)
+    cc = np.broadcast_to((1 << 20) + np.arange(n_lines * 4).reshape(1, n_lines, 4), (n, n_lines, 4))
+    u = _draws(kk.ravel(), cc.ravel()).reshape(n, n_lines, 4)
+    x = -0.5 * E + E * u[..., 0]; y = -0.5 * E + E * u[..., 1]
+    psi = -math.pi + 2.0 * math.pi * u[..., 2]
+    kappa = -0.03 + 0.06 * u[..., 3]
+    out = np.zeros((n, n_lines, pts_per_line, 2), dtype=np.float32)
+    for i in range(pts_per_line):
+        out[..., i, 0] = x; out[..., i, 1] = y
+        x = x + step * np.cos(psi); y = y + step * np.sin(psi)
+        psi = psi + kappa * step
+    return out
+
+
 def gen_dynamics(cfg: SceneConfig, world_begin: int = 0, n_worlds: int | None = None):
     """(speed[Wn][A] m/s, yaw_rate[Wn][A] rad/s) in float64 (G4)."""
     n = cfg.n_worlds - world_begin if n_worlds is None else n_worlds

@@ -66,8 +66,25 @@ def lib():
         L.orc_shadow_view.argtypes = [vp, ci, ci, cf, cf, vp, ctypes.POINTER(Params), ci, ci,
                                       vp, vp, vp, vp]
         L.orc_shadow_view.restype = ci
+        L.orc_polyline_quads.argtypes = [vp, ci, ci, cf, cf, ci, ci, vp]
+        L.orc_polyline_quads.restype = ci
         _lib = L
     return _lib
+
+
+def polyline_quads(points, half_width=0.075, z=0.01, cls=2, inst0=0, dtype=None):
+    """C1p: polylines [n_lines][pts][2] fp32 -> flat quads, one per segment (structured array of 48-byte
+    records; pass the generator's PRIM_DTYPE as `dtype`)."""
+    pts = np.ascontiguousarray(points, dtype=np.float32)
+    assert pts.ndim == 3 and pts.shape[2] == 2 and pts.shape[1] >= 2
+    n = pts.shape[0] * (pts.shape[1] - 1)
+    out = np.zeros(n, dtype=dtype if dtype is not None else np.dtype([("raw", "u1", (_PRIM_BYTES,))]))
+    assert out.dtype.itemsize == _PRIM_BYTES
+    rc = lib().orc_polyline_quads(pts.ctypes.data, pts.shape[0], pts.shape[1], float(half_width), float(z),
+                                  int(cls), int(inst0), out.ctypes.data)
+    if rc != n:
+        raise ValueError("orc_polyline_quads: bad arguments")
+    return out
 
 
 def _check_prims(prims):

@@ -325,3 +325,31 @@ int orc_shadow_view(const orc_prim *prims, int P, int ego, float cp_f, float sp_
     }
     return 0;
 }
+
+/* C1p: polyline -> thin planar strips (PAPER.md:62 "lane polylines ... thin planar strips", :331 "road
+ * geometry, encoded as polyline segments").  pts: [n_lines][pts_per_line][2] fp32 (x, y).  Segment s of
+ * line l becomes flat quad number q = l * (pts_per_line - 1) + s: centre at the segment's midpoint,
+ * half length along the segment, heading = the normalised segment direction (heading (1, 0) for a
+ * zero-length segment), half width / height / class as given, inst = inst0 + q.  fp32, one rounding
+ * per written operation (C1p).  Returns the number of quads written. */
+int orc_polyline_quads(const float *pts, int n_lines, int pts_per_line, float half_width, float z,
+                       int cls, int inst0, orc_prim *out)
+{
+    if (!pts || !out || n_lines < 0 || pts_per_line < 2) return -1;
+    int q = 0;
+    for (int l = 0; l < n_lines; ++l) {
+        for (int s = 0; s + 1 < pts_per_line; ++s, ++q) {
+            const float *p0 = pts + ((size_t)l * pts_per_line + s) * 2, *p1 = p0 + 2;
+            float dx = p1[0] - p0[0], dy = p1[1] - p0[1];
+            float len = sqrtf(fmaf(dy, dy, dx * dx));
+            float ck = 1.0f, sk = 0.0f;
+            if (len > 0.0f) { float inv = 1.0f / len; ck = dx * inv; sk = dy * inv; }
+            orc_prim *o = &out[q];
+            o->cx = fmaf(0.5f, dx, p0[0]); o->cy = fmaf(0.5f, dy, p0[1]); o->cz = z;
+            o->hx = 0.5f * len; o->hy = half_width; o->hz = 0.0f;
+            o->ck = ck; o->sk = sk;
+            o->cls = cls; o->inst = inst0 + q; o->shape = 0; o->pad1 = 0;
+        }
+    }
+    return q;
+}
