@@ -123,6 +123,17 @@ int gp_scene_upload(gp_ctx *ctx, const gp_scene_desc *desc, const gp_prim *h_age
  * aligned.  No host transfer. */
 int gp_agents_update(gp_ctx *ctx, const float *d_pose, void *stream);
 
+/* Static map from polylines, on the device (C1p; "lane polylines ... thin planar strips",
+ * :331 "road geometry, encoded as polyline segments").  d_points: DEVICE [Wn][n_lines][pts_per_line][2] fp32
+ * (x, y), 8-byte aligned.  Segment s of line l of world w overwrites static primitive number
+ * q = q_begin + l * (pts_per_line - 1) + s of that world (primitive A + q): a flat quad centred on the segment's
+ * midpoint, half length along the segment, heading = the normalised segment direction ((1, 0) for a zero-length
+ * segment), half width `half_width`, height `z`, class `cls`, instance A + q; its shading table is refreshed.
+ * q_begin >= 0 and q_begin + n_lines * (pts_per_line - 1) <= quads_per_world, pts_per_line >= 2.  No host
+ * transfer: a new map can be installed per episode without leaving the device. */
+int gp_statics_from_polylines(gp_ctx *ctx, const float *d_points, int n_lines, int pts_per_line,
+                              float half_width, float z, int cls, int q_begin, void *stream);
+
 /* Camera pitch per view.  d_pitch_cs: DEVICE [Wn][A][2] fp32 = (cos p, sin p), positive = nose up;
  * NULL resets every camera to pitch 0.  Copied on `stream`. */
 int gp_cameras_set(gp_ctx *ctx, const float *d_pitch_cs, void *stream);

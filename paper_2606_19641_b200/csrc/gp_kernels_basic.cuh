@@ -45,6 +45,31 @@ __global__ void k_agents_update(SceneConst sc, const float4 *__restrict__ pose, 
     write_meta(q, &meta[w * sc.P + a], sc);
 }
 
+// C1p: one thread per polyline segment -> flat quad record + its shading table.
+__global__ void k_polyline_quads(SceneConst sc, const float2 *__restrict__ pts, int n_lines, int pts_per_line,
+                                 float half_width, float z, int cls, int q_begin, gp_prim *__restrict__ prims,
+                                 PrimMeta *__restrict__ meta) {
+    const int segs = pts_per_line - 1, per_world = n_lines * segs;
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= (size_t)sc.Wn * per_world) return;
+    const int w = (int)(i / per_world), q = (int)(i % per_world);
+    const int l = q / segs, s = q - l * segs;
+    const float2 *p = pts + ((size_t)w * n_lines + l) * pts_per_line + s;
+    const float2 p0 = __ldg(p), p1 = __ldg(p + 1);
+    const float dx = c_sub(p1.x, p0.x), dy = c_sub(p1.y, p0.y);
+    const float len = c_sqrt(c_fma(dy, dy, c_mul(dx, dx)));
+    float ck = 1.0f, sk = 0.0f;
+    if (len > 0.0f) { const float inv = c_rcp(len); ck = c_mul(dx, inv); sk = c_mul(dy, inv); }
+    gp_prim o;
+    o.cx = c_fma(0.5f, dx, p0.x); o.cy = c_fma(0.5f, dy, p0.y); o.cz = z;
+    o.hx = c_mul(0.5f, len); o.hy = half_width; o.hz = 0.0f;
+    o.cos_yaw = ck; o.sin_yaw = sk;
+    o.cls = cls; o.inst = sc.A + q_begin + q; o.shape = GP_SHAPE_BOX; o.pad = 0;
+    const size_t k = (size_t)w * sc.P + sc.A + q_begin + q;
+    prims[k] = o;
+    write_meta(o, &meta[k], sc);
+}
+
 __global__ void k_fill_pitch(float2 *pitch, size_t n) {
     size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i < n) pitch[i] = make_float2(1.0f, 0.0f);

@@ -224,6 +224,23 @@ extern "C" int gp_agents_update(gp_ctx *c, const float *d_pose, void *stream_) {
     return GP_OK;
 }
 
+extern "C" int gp_statics_from_polylines(gp_ctx *c, const float *d_points, int n_lines, int pts_per_line,
+                                         float half_width, float z, int cls, int q_begin, void *stream_) {
+    if (!c || !d_points) return GP_ERR_ARG;
+    if (!c->have_scene) return GP_ERR_STATE;
+    if (n_lines < 1 || pts_per_line < 2 || cls < 0 || cls > 7 || !(half_width >= 0.0f)) return GP_ERR_ARG;
+    if (reinterpret_cast<uintptr_t>(d_points) & 7u) return GP_ERR_ALIGN;
+    const long long per_world = (long long)n_lines * (pts_per_line - 1);
+    if (q_begin < 0 || q_begin + per_world > c->sc.Q) return GP_ERR_RANGE;
+    const size_t n = (size_t)c->sc.Wn * (size_t)per_world;
+    k_polyline_quads<<<(unsigned)((n + 255) / 256), 256, 0, static_cast<cudaStream_t>(stream_)>>>(
+        c->sc, reinterpret_cast<const float2 *>(d_points), n_lines, pts_per_line, half_width, z, cls, q_begin,
+        c->d_prims, c->d_meta);
+    c->launches += 1;
+    CK(cudaGetLastError());
+    return GP_OK;
+}
+
 extern "C" int gp_cameras_set(gp_ctx *c, const float *d_pitch_cs, void *stream_) {
     if (!c) return GP_ERR_ARG;
     if (!c->have_scene) return GP_ERR_STATE;
