@@ -42,6 +42,7 @@ def parse():
     ap.add_argument("--worlds", type=int, default=0, help="override the number of worlds (debug)")
     ap.add_argument("--res", type=int, default=0, help="override H = W (resolution sweep)")
     ap.add_argument("--strip-px", type=int, default=0, help="GP_OPT_STRIP_PX override (0 = library default)")
+    ap.add_argument("--gather", type=int, default=-1, help="GP_OPT_GATHER override (-1 = library default)")
     ap.add_argument("--stage-cap", type=int, default=0, help="GP_OPT_STAGE_CAP override (0 = library default)")
     ap.add_argument("--chunk-worlds", type=int, default=0,
                     help="worlds per gp_render_batch call (0 = as many as keep the planes under 40 GB)")
@@ -205,6 +206,8 @@ def run_b200(args):
         r.set_option(gp.GP_OPT_STRIP_PX, args.strip_px)
     if args.stage_cap:
         r.set_option(gp.GP_OPT_STAGE_CAP, args.stage_cap)
+    if args.gather >= 0:
+        r.set_option(gp.GP_OPT_GATHER, args.gather)
     r.scene_upload(agents, quads, cam_height=cfg.cam_height, t_max=cfg.t_max)
     if cfg.pitch_deg_max > 0:
         r.cameras_set(torch.from_numpy(gs.gen_pitch(big, w0, cfg.n_worlds)).to(dev))

@@ -47,7 +47,10 @@ enum {
     GP_OPT_TIMING = 3,      /* 1: bracket every kernel launch with CUDA events (gp_kernel_time) */
     GP_OPT_STAGE_CAP = 4,   /* list entries per view staged in shared memory (default 128, >= 1);
                                longer lists read their tail from global memory                  */
-    GP_OPT_STRIP_PX = 5     /* target pixels per warp strip of the render pass; 0 = automatic   */
+    GP_OPT_STRIP_PX = 5,    /* target pixels per warp strip of the render pass; 0 = automatic   */
+    GP_OPT_GATHER = 6       /* how a strip works off its list: 1 gather the overlapping entries first, one lane
+                               per (flat quad, row); 0 entry by entry; -1 (default) chosen from the image size
+                               and the primitives per world                                        */
 };
 enum {                      /* kernel ids of gp_kernel_time                                   */
     GP_KERNEL_UPDATE = 0,   /* a0 pose update + shading table                                 */

@@ -158,6 +158,7 @@ __device__ __forceinline__ void slab_z(const float4 &g1, const float4 &rt, float
     const float ta = c_mul(g1.x, rt.z), tb = c_mul(g1.y, rt.z);
     loz = c_min(ta, tb); hiz = c_max(ta, tb);
 }
+template <bool ATOMIC>      // ATOMIC: other lanes of the warp may update the same key at the same time
 __device__ __forceinline__ void slab_select(const float4 &g0, float dlx, float dly, float loz, float hiz, float dz,
                                             float t_max, bool flat, uint32_t klow, unsigned long long *kp) {
     const float ix = c_rcp(dlx), iy = c_rcp(dly);
@@ -175,8 +176,191 @@ __device__ __forceinline__ void slab_select(const float4 &g0, float dlx, float d
         else if (loy == tn) face = 2 + (dly > 0.0f ? 0 : 1);
         else face = 4 + (dz > 0.0f ? 0 : 1);
         const unsigned long long key = ((unsigned long long)__float_as_uint(tn) << 32) | klow | face;   // C6
-        if (key < *kp) *kp = key;
+        if (ATOMIC) atomicMin(kp, key);
+        else if (key < *kp) *kp = key;
     }
+}
+
+// ---- a6 / a7 for one strip -------------------------------------------------------------------------
+constexpr int kOverlapCap = 64;      // entries of one strip worked off per batch (per-warp overlap list)
+#ifndef GP_SHORT_SPAN
+#define GP_SHORT_SPAN 3
+#endif
+constexpr int kShortSpan = GP_SHORT_SPAN;   // flat-quad column spans up to this many pixels are finished by their own lane
+
+struct StripBatchCtx {
+    const EntryGeo *s_geo, *g_geo; const EntryAux *s_aux, *g_aux;
+    const float4 *s_row; const float *s_col;
+    int scap, W, log2LC;
+    float th, t_max;
+};
+struct EntryRec { float4 g0, g1, g2; uint4 ax; };   // (ax bx ay by) (az bz flx fly) (rlx rly ulx uly) aux
+
+__device__ __forceinline__ EntryRec load_entry(const StripBatchCtx &c, int eb) {
+    EntryRec r;
+    if (eb < c.scap) {
+        const float4 *sg = reinterpret_cast<const float4 *>(&c.s_geo[eb]);
+        r.g0 = sg[0]; r.g1 = sg[1]; r.g2 = sg[2];
+        r.ax = *reinterpret_cast<const uint4 *>(&c.s_aux[eb]);
+    } else {                            // rare: list longer than the staged capacity
+        const float4 *gg = reinterpret_cast<const float4 *>(&c.g_geo[eb]);
+        r.g0 = __ldg(gg); r.g1 = __ldg(gg + 1); r.g2 = __ldg(gg + 2);
+        r.ax = __ldg(reinterpret_cast<const uint4 *>(&c.g_aux[eb]));
+    }
+    return r;
+}
+
+// Conservative column interval [ja, jb] of a flat entry on the row with table entry rt (not contract
+// arithmetic: plain fp32 + slack): the plane depth t is fixed per row, so the footprint is one interval.
+__device__ __forceinline__ void flat_interval(const EntryRec &E, const float4 &rt, const StripBatchCtx &c, int &ja, int &jb) {
+    const float4 &g0 = E.g0, &g1 = E.g1, &g2 = E.g2;
+    const int c0 = (int)(E.ax.z & 0xffff), c1 = (int)(E.ax.z >> 16);
+    ja = 1; jb = 0;
+    // centre -ol and half extents h in the ray-origin frame, recovered from a = -h - ol, b = h - ol
+    const float mx = 0.5f * (g0.x + g0.y), my = 0.5f * (g0.z + g0.w), mz = 0.5f * (g1.x + g1.y);
+    const float ex_ = 0.5f * (g0.y - g0.x), ey_ = 0.5f * (g0.w - g0.z);
+    const float dl_ = 2e-5f * (fabsf(mx) + fabsf(my) + fabsf(mz) + ex_ + ey_) + 1e-6f;
+    const float hxs = ex_ + dl_, hys = ey_ + dl_;
+    const float t = g1.x * rt.z;                     // plane depth on this row
+    if (!(t > 0.0f && t <= c.t_max * 1.00001f)) return;
+    const float X0 = fmaf(t, fmaf(rt.x, g2.z, g1.z), -mx), X1 = t * g2.x;
+    const float Y0 = fmaf(t, fmaf(rt.x, g2.w, g1.w), -my), Y1 = t * g2.y;
+    float slo = -3.0e38f, shi = 3.0e38f;
+    bool ok = true;
+    if (fabsf(X1) > 1e-12f) {
+        const float r = flat_rcp(X1), a = (-hxs - X0) * r, b = (hxs - X0) * r;
+        slo = fmaxf(slo, fminf(a, b)); shi = fminf(shi, fmaxf(a, b));
+    } else ok = fabsf(X0) <= hxs;
+    if (fabsf(Y1) > 1e-12f) {
+        const float r = flat_rcp(Y1), a = (-hys - Y0) * r, b = (hys - Y0) * r;
+        slo = fmaxf(slo, fminf(a, b)); shi = fminf(shi, fmaxf(a, b));
+    } else ok = ok && fabsf(Y0) <= hys;
+    if (!(ok && slo <= shi)) return;
+    // column of s: (s/th + 1) W/2 - 0.5, widened by 0.02 px + relative slack
+    const float col_scale = 0.5f * (float)c.W / c.th;
+    const float xa = fmaf(slo, col_scale, 0.5f * (float)c.W - 0.52f) - 1e-5f * fabsf(slo * col_scale);
+    const float xb = fmaf(shi, col_scale, 0.5f * (float)c.W - 0.48f) + 1e-5f * fabsf(shi * col_scale);
+    ja = max(c0, (int)ceilf(fmaxf(xa, -1.0f)));
+    jb = min(c1, (int)floorf(fminf(xb, (float)c.W)));
+}
+
+// The gathered entries of one strip: olist[0 .. nfl) flat quads, olist[kOverlapCap - nbx .. kOverlapCap) boxes and
+// spheres.  Flat quads: one lane per (entry, row) bounds the row's column interval; a short interval is finished
+// by that lane (atomic minimum: two lanes may meet on a pixel), a long one is spread over the warp afterwards.
+// Boxes / spheres: the warp spreads over the entry's pixel rectangle inside the strip.  Returns the number of
+// exact tests (STATS only).
+template <bool STATS, bool SPH>
+__device__ __forceinline__ unsigned strip_batch(const StripBatchCtx &c, const uint16_t *olist, int nfl, int nbx,
+                                                int row0, int row1, unsigned long long *keys, int lane) {
+    unsigned n_tests = 0;
+    const int W = c.W;
+    const float t_max = c.t_max;
+    const int nrows = row1 - row0 + 1;
+    // ---- flat quads -------------------------------------------------------------------------------
+    const int nitems = nfl * nrows;
+    const bool pow2 = (nrows & (nrows - 1)) == 0;             // rows per strip: a power of two except in a ragged last strip
+    const int sh = 31 - __clz(nrows);
+    for (int t0 = 0; t0 < nitems; t0 += 32) {
+        const int t = t0 + lane;
+        int ja = 1, jb = 0, i = row0, eb = 0;
+        uint32_t klow = 0;
+        if (t < nitems) {
+            const int le = pow2 ? t >> sh : t / nrows;
+            i = row0 + (t - le * nrows);
+            eb = olist[le];
+            const EntryRec E = load_entry(c, eb);
+            klow = (E.ax.x >> 2) << 3;
+            if (i >= (int)(E.ax.y & 0xffff) && i <= (int)(E.ax.y >> 16)) {
+                const float4 rt = c.s_row[i];
+                const int c0 = (int)(E.ax.z & 0xffff), c1 = (int)(E.ax.z >> 16);
+                if (c1 - c0 < kShortSpan) { ja = c0; jb = c1; }    // a few columns only: not worth bounding further
+                else flat_interval(E, rt, c, ja, jb);
+                if (jb - ja < kShortSpan) {                        // short (or empty): finish it here
+                    float loz, hiz;
+                    slab_z(E.g1, rt, loz, hiz);
+                    unsigned long long *krow = keys + (i - row0) * W;
+                    for (int j = ja; j <= jb; ++j) {
+                        if (STATS) ++n_tests;
+                        const float s = c.s_col[j];
+                        const float dlx = c_fma(rt.x, E.g2.z, c_fma(s, E.g2.x, E.g1.z));
+                        const float dly = c_fma(rt.x, E.g2.w, c_fma(s, E.g2.y, E.g1.w));
+                        slab_select<true>(E.g0, dlx, dly, loz, hiz, rt.y, t_max, true, klow, krow + j);
+                    }
+                    jb = ja - 1;                                   // done
+                }
+            }
+        }
+        __syncwarp();
+        unsigned lm = __ballot_sync(0xffffffffu, jb >= ja);        // long spans: all lanes, one item at a time
+        while (lm) {
+            const int src = __ffs(lm) - 1;
+            lm &= lm - 1;
+            const int bi = __shfl_sync(0xffffffffu, i, src), beb = __shfl_sync(0xffffffffu, eb, src);
+            const int bja = __shfl_sync(0xffffffffu, ja, src), bjb = __shfl_sync(0xffffffffu, jb, src);
+            const EntryRec E = load_entry(c, beb);
+            const uint32_t bk = (E.ax.x >> 2) << 3;
+            const float4 rt = c.s_row[bi];
+            float loz, hiz;
+            slab_z(E.g1, rt, loz, hiz);
+            unsigned long long *krow = keys + (bi - row0) * W;
+            for (int j = bja + lane; j <= bjb; j += 32) {
+                if (STATS) ++n_tests;
+                const float s = c.s_col[j];
+                const float dlx = c_fma(rt.x, E.g2.z, c_fma(s, E.g2.x, E.g1.z));
+                const float dly = c_fma(rt.x, E.g2.w, c_fma(s, E.g2.y, E.g1.w));
+                slab_select<false>(E.g0, dlx, dly, loz, hiz, rt.y, t_max, true, bk, krow + j);
+            }
+            __syncwarp();
+        }
+    }
+    // ---- boxes and spheres ------------------------------------------------------------------------
+    const int LC = 1 << c.log2LC, LR = 32 >> c.log2LC;
+    const int li = lane >> c.log2LC, lj = lane & (LC - 1);
+    for (int ib = 0; ib < nbx; ++ib) {
+        const EntryRec E = load_entry(c, olist[kOverlapCap - 1 - ib]);
+        const float4 &g0 = E.g0, &g1 = E.g1, &g2 = E.g2;
+        const uint32_t kind = E.ax.x & 3u, klow = (E.ax.x >> 2) << 3;
+        const int r0 = max((int)(E.ax.y & 0xffff), row0), r1 = min((int)(E.ax.y >> 16), row1);
+        const int c0 = (int)(E.ax.z & 0xffff), c1 = (int)(E.ax.z >> 16);
+        for (int rb = r0; rb <= r1; rb += LR) {
+            const int i = min(rb + li, r1);                         // lanes past r1 idle (j loop below)
+            const bool row_ok = rb + li <= r1;
+            const float4 rt = c.s_row[i];                           // v, dz, 1/dz, tg
+            unsigned long long *krow = keys + (i - row0) * W;
+            if (SPH && kind == kKindSphere) {
+                // C5s over the entry's pixel rectangle; g0 = (e.x, e.y, e.z, r*r), basis = world frame
+                for (int cb = c0; cb <= c1; cb += LC) {
+                    const int j = cb + lj;
+                    if (row_ok && j <= c1) {
+                        if (STATS) ++n_tests;
+                        const float s = c.s_col[j];
+                        const float dx = c_fma(rt.x, g2.z, c_fma(s, g2.x, g1.z));
+                        const float dy = c_fma(rt.x, g2.w, c_fma(s, g2.y, g1.w));
+                        const float tn = sphere_entry(g0.x, g0.y, g0.z, g0.w, dx, dy, rt.y);
+                        if (tn > 0.0f && tn <= t_max) {
+                            const unsigned long long key = ((unsigned long long)__float_as_uint(tn) << 32) | klow | 5u;
+                            if (key < krow[j]) krow[j] = key;
+                        }
+                    }
+                }
+            } else {
+                float loz, hiz;
+                slab_z(g1, rt, loz, hiz);                           // per row, not per pixel
+                for (int cb = c0; cb <= c1; cb += LC) {
+                    const int j = cb + lj;
+                    if (row_ok && j <= c1) {
+                        if (STATS) ++n_tests;
+                        const float s = c.s_col[j];
+                        const float dlx = c_fma(rt.x, g2.z, c_fma(s, g2.x, g1.z));      // C5, per-pixel part
+                        const float dly = c_fma(rt.x, g2.w, c_fma(s, g2.y, g1.w));
+                        slab_select<false>(g0, dlx, dly, loz, hiz, rt.y, t_max, false, klow, krow + j);
+                    }
+                }
+            }
+        }
+        __syncwarp();
+    }
+    return n_tests;
 }
 
 #ifndef GP_RENDER_WARPS
@@ -187,7 +371,11 @@ __device__ __forceinline__ void slab_select(const float4 &g0, float dlx, float d
 #endif
 // NG: 128-pixel groups per strip when W is a power of two (1, 2, 4), else 0.  SPH: the scene holds spheres
 // (scenes without any run the variant compiled without the C5s branch: it costs the strip loop registers).
-template <bool STATS, int NG, bool SPH>
+// GATHER: how a strip works off its list.  true: the overlapping entries are first gathered into a per-warp list and
+// flat quads get one lane per (entry, row) (fewer instructions when many entries meet a strip: small images, dense
+// scenes); false: entry by entry as the ballot finds them, the warp spread over each entry's rectangle (1 % faster
+// when lists are short and the kernel is store-bound).  The host picks (gp_lib.cu).
+template <bool STATS, int NG, bool SPH, bool GATHER>
 __global__ void __launch_bounds__(GP_RENDER_WARPS * 32, GP_RENDER_MIN_CTAS)
 k_render(SceneConst sc, RenderArgs ra) {
     extern __shared__ __align__(16) unsigned char smem[];
@@ -202,7 +390,8 @@ k_render(SceneConst sc, RenderArgs ra) {
     EntryAux *s_aux = reinterpret_cast<EntryAux *>(smem + 48 + (size_t)ra.scap * 48);
     float4 *s_row = reinterpret_cast<float4 *>(smem + 48 + (size_t)ra.scap * 64);
     float *s_col = reinterpret_cast<float *>(s_row + H);
-    unsigned long long *s_keys = reinterpret_cast<unsigned long long *>(s_col + ((W + 3) & ~3));
+    uint16_t *s_olist = reinterpret_cast<uint16_t *>(s_col + ((W + 3) & ~3));          // [warps][kOverlapCap], GATHER only
+    unsigned long long *s_keys = reinterpret_cast<unsigned long long *>(s_olist + (GATHER ? (blockDim.x >> 5) * kOverlapCap : 0));
     unsigned long long *keys = s_keys + (size_t)warp * SR * W;
 
     const float4 vh4 = __ldg(reinterpret_cast<const float4 *>(&ra.hdr[view]));
@@ -243,14 +432,11 @@ k_render(SceneConst sc, RenderArgs ra) {
 
     const int w = ra.world_begin + view / (sc.A * sc.C);
     const uint32_t *wtab = reinterpret_cast<const uint32_t *>(ra.meta + (size_t)w * sc.P);   // uint32[P][8]
-    const int LC = 1 << ra.log2LC, LR = 32 >> ra.log2LC;
-    const int li = lane >> ra.log2LC, lj = lane & (LC - 1);
     const size_t HW = (size_t)H * W;
     const int n_strips = (H + SR - 1) / SR;
     // resolve pass: lane owns pixels 4*lane .. 4*lane+3 of every 128-pixel group of the strip
     const int lane_row = (lane * 4) / W, lane_col = (lane * 4) % W;
     const int step_row = 128 / W, step_col = 128 % W;
-    const float t_max = sc.t_max;
     unsigned long long n_tests = 0;
 
     // Strip schedule: strips are handed out dynamically in ascending order (ascending addresses are
@@ -269,135 +455,180 @@ k_render(SceneConst sc, RenderArgs ra) {
         const int nn = strip < n_free ? 0 : n;                      // entries to scan for this strip
         const int row0 = strip * SR, row1 = min(H, row0 + SR) - 1;
         bool any = false;
-        // ---- a3: warp-level early-out over the list, a6/a7: slab test + select ----------------
-        for (int base = 0; base < nn; base += 32) {
-            const int e = base + lane;
-            bool ov = false;
-            if (e < nn) {
-                const uint32_t rows = e < ra.scap ? s_aux[e].rows : __ldg(&g_aux[e].rows);
-                ov = (int)(rows & 0xffff) <= row1 && (int)(rows >> 16) >= row0;
-            }
-            unsigned mask = __ballot_sync(0xffffffffu, ov);
-            if (mask && !any) {
-                any = true;
-                ulonglong2 *k2 = reinterpret_cast<ulonglong2 *>(keys);
-                const int nk2 = (row1 - row0 + 1) * W / 2;
-                for (int q = lane; q < nk2; q += 32) k2[q] = make_ulonglong2(kKeyEmpty, kKeyEmpty);
-                __syncwarp();
-            }
-            while (mask) {
-                const int eb = base + __ffs(mask) - 1;
-                mask &= mask - 1;
-                float4 g0, g1, g2; uint4 ax;        // (ax bx ay by) (az bz flx fly) (rlx rly ulx uly) aux
-                if (eb < ra.scap) {
-                    const float4 *sg = reinterpret_cast<const float4 *>(&s_geo[eb]);
-                    g0 = sg[0]; g1 = sg[1]; g2 = sg[2];
-                    ax = *reinterpret_cast<const uint4 *>(&s_aux[eb]);
-                } else {                            // rare: list longer than the staged capacity
-                    const float4 *gg = reinterpret_cast<const float4 *>(&g_geo[eb]);
-                    g0 = __ldg(gg); g1 = __ldg(gg + 1); g2 = __ldg(gg + 2);
-                    ax = __ldg(reinterpret_cast<const uint4 *>(&g_aux[eb]));
+        if (GATHER) {
+            const unsigned lt_mask = (1u << lane) - 1u;
+            uint16_t *olist = s_olist + warp * kOverlapCap;
+            StripBatchCtx sb;
+            sb.s_geo = s_geo; sb.g_geo = g_geo; sb.s_aux = s_aux; sb.g_aux = g_aux;
+            sb.s_row = s_row; sb.s_col = s_col; sb.scap = ra.scap; sb.W = W; sb.log2LC = ra.log2LC; sb.th = ra.th; sb.t_max = sc.t_max;
+            // ---- a3: warp-level early-out over the list: the entries whose rows overlap the strip are gathered
+            // (ballot) into the warp's overlap list, flat quads from the front, boxes / spheres from the back;
+            // a6/a7 then run per batch in strip_batch().
+            int nfl = 0, nbx = 0;
+            for (int base = 0; base < nn; base += 32) {
+                const int e = base + lane;
+                bool ov = false, fl = false;
+                if (e < nn) {
+                    const uint2 kr = e < ra.scap ? *reinterpret_cast<const uint2 *>(&s_aux[e])
+                                                 : __ldg(reinterpret_cast<const uint2 *>(&g_aux[e]));   // kf, rows
+                    ov = (int)(kr.y & 0xffff) <= row1 && (int)(kr.y >> 16) >= row0;
+                    fl = (kr.x & 3u) == kKindFlat;
                 }
-                const uint32_t kind = ax.x & 3u;
-                const bool flat = kind == kKindFlat;
-                const uint32_t klow = (ax.x >> 2) << 3;
-                const int r0 = max((int)(ax.y & 0xffff), row0), r1 = min((int)(ax.y >> 16), row1);
-                const int c0 = (int)(ax.z & 0xffff), c1 = (int)(ax.z >> 16);
-                if (SPH && kind == kKindSphere) {
-                    // C5s over the entry's pixel rectangle; g0 = (e.x, e.y, e.z, r*r), basis = world frame
-                    for (int rb = r0; rb <= r1; rb += LR) {
-                        const int i = rb + li;
-                        for (int cb = c0; cb <= c1; cb += LC) {
-                            const int j = cb + lj;
-                            if (i <= r1 && j <= c1) {
-                                if (STATS) ++n_tests;
-                                const float s = s_col[j];
-                                const float4 rt = s_row[i];
-                                const float dx = c_fma(rt.x, g2.z, c_fma(s, g2.x, g1.z));
-                                const float dy = c_fma(rt.x, g2.w, c_fma(s, g2.y, g1.w));
-                                const float tn = sphere_entry(g0.x, g0.y, g0.z, g0.w, dx, dy, rt.y);
-                                if (tn > 0.0f && tn <= t_max) {
-                                    const unsigned long long key = ((unsigned long long)__float_as_uint(tn) << 32) | klow | 5u;
-                                    unsigned long long *kp = &keys[(i - row0) * W + j];
-                                    if (key < *kp) *kp = key;
+                const unsigned fmask = __ballot_sync(0xffffffffu, ov && fl), bmask = __ballot_sync(0xffffffffu, ov && !fl);
+                if (!(fmask | bmask)) continue;
+                if (!any) {
+                    any = true;
+                    ulonglong2 *k2 = reinterpret_cast<ulonglong2 *>(keys);
+                    const int nk2 = (row1 - row0 + 1) * W / 2;
+                    for (int q = lane; q < nk2; q += 32) k2[q] = make_ulonglong2(kKeyEmpty, kKeyEmpty);
+                }
+                if (nfl + nbx + __popc(fmask) + __popc(bmask) > kOverlapCap) {       // no room: work off what is gathered
+                    __syncwarp();
+                    n_tests += strip_batch<STATS, SPH>(sb, olist, nfl, nbx, row0, row1, keys, lane);
+                    nfl = nbx = 0;
+                }
+                if (ov && fl) olist[nfl + __popc(fmask & lt_mask)] = (uint16_t)e;
+                if (ov && !fl) olist[kOverlapCap - 1 - (nbx + __popc(bmask & lt_mask))] = (uint16_t)e;
+                nfl += __popc(fmask); nbx += __popc(bmask);
+            }
+            if (nfl + nbx) {
+                __syncwarp();
+                n_tests += strip_batch<STATS, SPH>(sb, olist, nfl, nbx, row0, row1, keys, lane);
+            }
+        } else {
+            const int LC = 1 << ra.log2LC, LR = 32 >> ra.log2LC;
+            const int li = lane >> ra.log2LC, lj = lane & (LC - 1);
+            const float t_max = sc.t_max;
+            // ---- a3: warp-level early-out over the list, a6/a7: slab test + select ----------------
+            for (int base = 0; base < nn; base += 32) {
+                const int e = base + lane;
+                bool ov = false;
+                if (e < nn) {
+                    const uint32_t rows = e < ra.scap ? s_aux[e].rows : __ldg(&g_aux[e].rows);
+                    ov = (int)(rows & 0xffff) <= row1 && (int)(rows >> 16) >= row0;
+                }
+                unsigned mask = __ballot_sync(0xffffffffu, ov);
+                if (mask && !any) {
+                    any = true;
+                    ulonglong2 *k2 = reinterpret_cast<ulonglong2 *>(keys);
+                    const int nk2 = (row1 - row0 + 1) * W / 2;
+                    for (int q = lane; q < nk2; q += 32) k2[q] = make_ulonglong2(kKeyEmpty, kKeyEmpty);
+                    __syncwarp();
+                }
+                while (mask) {
+                    const int eb = base + __ffs(mask) - 1;
+                    mask &= mask - 1;
+                    float4 g0, g1, g2; uint4 ax;        // (ax bx ay by) (az bz flx fly) (rlx rly ulx uly) aux
+                    if (eb < ra.scap) {
+                        const float4 *sg = reinterpret_cast<const float4 *>(&s_geo[eb]);
+                        g0 = sg[0]; g1 = sg[1]; g2 = sg[2];
+                        ax = *reinterpret_cast<const uint4 *>(&s_aux[eb]);
+                    } else {                            // rare: list longer than the staged capacity
+                        const float4 *gg = reinterpret_cast<const float4 *>(&g_geo[eb]);
+                        g0 = __ldg(gg); g1 = __ldg(gg + 1); g2 = __ldg(gg + 2);
+                        ax = __ldg(reinterpret_cast<const uint4 *>(&g_aux[eb]));
+                    }
+                    const uint32_t kind = ax.x & 3u;
+                    const bool flat = kind == kKindFlat;
+                    const uint32_t klow = (ax.x >> 2) << 3;
+                    const int r0 = max((int)(ax.y & 0xffff), row0), r1 = min((int)(ax.y >> 16), row1);
+                    const int c0 = (int)(ax.z & 0xffff), c1 = (int)(ax.z >> 16);
+                    if (SPH && kind == kKindSphere) {
+                        // C5s over the entry's pixel rectangle; g0 = (e.x, e.y, e.z, r*r), basis = world frame
+                        for (int rb = r0; rb <= r1; rb += LR) {
+                            const int i = rb + li;
+                            for (int cb = c0; cb <= c1; cb += LC) {
+                                const int j = cb + lj;
+                                if (i <= r1 && j <= c1) {
+                                    if (STATS) ++n_tests;
+                                    const float s = s_col[j];
+                                    const float4 rt = s_row[i];
+                                    const float dx = c_fma(rt.x, g2.z, c_fma(s, g2.x, g1.z));
+                                    const float dy = c_fma(rt.x, g2.w, c_fma(s, g2.y, g1.w));
+                                    const float tn = sphere_entry(g0.x, g0.y, g0.z, g0.w, dx, dy, rt.y);
+                                    if (tn > 0.0f && tn <= t_max) {
+                                        const unsigned long long key = ((unsigned long long)__float_as_uint(tn) << 32) | klow | 5u;
+                                        unsigned long long *kp = &keys[(i - row0) * W + j];
+                                        if (key < *kp) *kp = key;
+                                    }
+                                }
+                            }
+                        }
+                    } else if (flat && c1 - c0 >= LC) {
+                        // Wide flat primitive: per row, the plane depth t is fixed, so the footprint is one
+                        // column interval.  Bound it conservatively (plain fp32 + slack) and run the exact
+                        // test only inside it: a thin diagonal marking costs ~its length, not its bbox area.
+                        // (not contract arithmetic: centre -ol and half extents h in the ray-origin frame, recovered from
+                        // a = -h - ol, b = h - ol)
+                        const float mx = 0.5f * (g0.x + g0.y), my = 0.5f * (g0.z + g0.w), mz = 0.5f * (g1.x + g1.y);
+                        const float ex_ = 0.5f * (g0.y - g0.x), ey_ = 0.5f * (g0.w - g0.z);
+                        const float dl_ = 2e-5f * (fabsf(mx) + fabsf(my) + fabsf(mz) + ex_ + ey_) + 1e-6f;
+                        const float hxs = ex_ + dl_, hys = ey_ + dl_;
+                        const float col_scale = 0.5f * (float)W / ra.th;
+                        for (int rb = r0; rb <= r1; rb += LR) {
+                            const int i = rb + li;
+                            int ja = 1, jb = 0;                                  // empty
+                            float4 rt = make_float4(0.f, 0.f, 0.f, 0.f);
+                            if (i <= r1) {
+                                rt = s_row[i];
+                                const float t = g1.x * rt.z;                     // plane depth on this row
+                                if (t > 0.0f && t <= t_max * 1.00001f) {
+                                    const float X0 = fmaf(t, fmaf(rt.x, g2.z, g1.z), -mx), X1 = t * g2.x;
+                                    const float Y0 = fmaf(t, fmaf(rt.x, g2.w, g1.w), -my), Y1 = t * g2.y;
+                                    float slo = -3.0e38f, shi = 3.0e38f;
+                                    bool ok = true;
+                                    if (fabsf(X1) > 1e-12f) {
+                                        const float r = flat_rcp(X1), a = (-hxs - X0) * r, b = (hxs - X0) * r;
+                                        slo = fmaxf(slo, fminf(a, b)); shi = fminf(shi, fmaxf(a, b));
+                                    } else ok = fabsf(X0) <= hxs;
+                                    if (fabsf(Y1) > 1e-12f) {
+                                        const float r = flat_rcp(Y1), a = (-hys - Y0) * r, b = (hys - Y0) * r;
+                                        slo = fmaxf(slo, fminf(a, b)); shi = fminf(shi, fmaxf(a, b));
+                                    } else ok = ok && fabsf(Y0) <= hys;
+                                    if (ok && slo <= shi) {
+                                        // column of s: (s/th + 1) W/2 - 0.5, widened by 0.02 px + relative slack
+                                        const float xa = fmaf(slo, col_scale, 0.5f * (float)W - 0.52f) - 1e-5f * fabsf(slo * col_scale);
+                                        const float xb = fmaf(shi, col_scale, 0.5f * (float)W - 0.48f) + 1e-5f * fabsf(shi * col_scale);
+                                        ja = max(c0, (int)ceilf(fmaxf(xa, -1.0f)));
+                                        jb = min(c1, (int)floorf(fminf(xb, (float)W)));
+                                    }
+                                }
+                            }
+                            float loz, hiz;
+                            slab_z(g1, rt, loz, hiz);
+                            unsigned long long *krow = keys + (i - row0) * W;
+                            for (int j = ja + lj; __any_sync(0xffffffffu, j <= jb); j += LC) {
+                                if (j <= jb) {
+                                    if (STATS) ++n_tests;
+                                    const float s = s_col[j];
+                                    const float dlx = c_fma(rt.x, g2.z, c_fma(s, g2.x, g1.z));
+                                    const float dly = c_fma(rt.x, g2.w, c_fma(s, g2.y, g1.w));
+                                    slab_select<false>(g0, dlx, dly, loz, hiz, rt.y, t_max, true, klow, krow + j);
+                                }
+                            }
+                        }
+                    } else {
+                        for (int rb = r0; rb <= r1; rb += LR) {
+                            const int i = min(rb + li, r1);                         // lanes past r1 idle (j loop below)
+                            const bool row_ok = rb + li <= r1;
+                            const float4 rt = s_row[i];                             // v, dz, 1/dz, tg
+                            float loz, hiz;
+                            slab_z(g1, rt, loz, hiz);                               // per row, not per pixel
+                            unsigned long long *krow = keys + (i - row0) * W;
+                            for (int cb = c0; cb <= c1; cb += LC) {
+                                const int j = cb + lj;
+                                if (row_ok && j <= c1) {
+                                    if (STATS) ++n_tests;
+                                    const float s = s_col[j];
+                                    const float dlx = c_fma(rt.x, g2.z, c_fma(s, g2.x, g1.z));
+                                    const float dly = c_fma(rt.x, g2.w, c_fma(s, g2.y, g1.w));
+                                    slab_select<false>(g0, dlx, dly, loz, hiz, rt.y, t_max, flat, klow, krow + j);
                                 }
                             }
                         }
                     }
-                } else if (flat && c1 - c0 >= LC) {
-                    // Wide flat primitive: per row, the plane depth t is fixed, so the footprint is one
-                    // column interval.  Bound it conservatively (plain fp32 + slack) and run the exact
-                    // test only inside it: a thin diagonal marking costs ~its length, not its bbox area.
-                    // (not contract arithmetic: centre -ol and half extents h in the ray-origin frame, recovered from
-                    // a = -h - ol, b = h - ol)
-                    const float mx = 0.5f * (g0.x + g0.y), my = 0.5f * (g0.z + g0.w), mz = 0.5f * (g1.x + g1.y);
-                    const float ex_ = 0.5f * (g0.y - g0.x), ey_ = 0.5f * (g0.w - g0.z);
-                    const float dl_ = 2e-5f * (fabsf(mx) + fabsf(my) + fabsf(mz) + ex_ + ey_) + 1e-6f;
-                    const float hxs = ex_ + dl_, hys = ey_ + dl_;
-                    const float col_scale = 0.5f * (float)W / ra.th;
-                    for (int rb = r0; rb <= r1; rb += LR) {
-                        const int i = rb + li;
-                        int ja = 1, jb = 0;                                  // empty
-                        float4 rt = make_float4(0.f, 0.f, 0.f, 0.f);
-                        if (i <= r1) {
-                            rt = s_row[i];
-                            const float t = g1.x * rt.z;                     // plane depth on this row
-                            if (t > 0.0f && t <= t_max * 1.00001f) {
-                                const float X0 = fmaf(t, fmaf(rt.x, g2.z, g1.z), -mx), X1 = t * g2.x;
-                                const float Y0 = fmaf(t, fmaf(rt.x, g2.w, g1.w), -my), Y1 = t * g2.y;
-                                float slo = -3.0e38f, shi = 3.0e38f;
-                                bool ok = true;
-                                if (fabsf(X1) > 1e-12f) {
-                                    const float r = flat_rcp(X1), a = (-hxs - X0) * r, b = (hxs - X0) * r;
-                                    slo = fmaxf(slo, fminf(a, b)); shi = fminf(shi, fmaxf(a, b));
-                                } else ok = fabsf(X0) <= hxs;
-                                if (fabsf(Y1) > 1e-12f) {
-                                    const float r = flat_rcp(Y1), a = (-hys - Y0) * r, b = (hys - Y0) * r;
-                                    slo = fmaxf(slo, fminf(a, b)); shi = fminf(shi, fmaxf(a, b));
-                                } else ok = ok && fabsf(Y0) <= hys;
-                                if (ok && slo <= shi) {
-                                    // column of s: (s/th + 1) W/2 - 0.5, widened by 0.02 px + relative slack
-                                    const float xa = fmaf(slo, col_scale, 0.5f * (float)W - 0.52f) - 1e-5f * fabsf(slo * col_scale);
-                                    const float xb = fmaf(shi, col_scale, 0.5f * (float)W - 0.48f) + 1e-5f * fabsf(shi * col_scale);
-                                    ja = max(c0, (int)ceilf(fmaxf(xa, -1.0f)));
-                                    jb = min(c1, (int)floorf(fminf(xb, (float)W)));
-                                }
-                            }
-                        }
-                        float loz, hiz;
-                        slab_z(g1, rt, loz, hiz);
-                        unsigned long long *krow = keys + (i - row0) * W;
-                        for (int j = ja + lj; __any_sync(0xffffffffu, j <= jb); j += LC) {
-                            if (j <= jb) {
-                                if (STATS) ++n_tests;
-                                const float s = s_col[j];
-                                const float dlx = c_fma(rt.x, g2.z, c_fma(s, g2.x, g1.z));
-                                const float dly = c_fma(rt.x, g2.w, c_fma(s, g2.y, g1.w));
-                                slab_select(g0, dlx, dly, loz, hiz, rt.y, t_max, true, klow, krow + j);
-                            }
-                        }
-                    }
-                } else {
-                    for (int rb = r0; rb <= r1; rb += LR) {
-                        const int i = min(rb + li, r1);                         // lanes past r1 idle (j loop below)
-                        const bool row_ok = rb + li <= r1;
-                        const float4 rt = s_row[i];                             // v, dz, 1/dz, tg
-                        float loz, hiz;
-                        slab_z(g1, rt, loz, hiz);                               // per row, not per pixel
-                        unsigned long long *krow = keys + (i - row0) * W;
-                        for (int cb = c0; cb <= c1; cb += LC) {
-                            const int j = cb + lj;
-                            if (row_ok && j <= c1) {
-                                if (STATS) ++n_tests;
-                                const float s = s_col[j];
-                                const float dlx = c_fma(rt.x, g2.z, c_fma(s, g2.x, g1.z));
-                                const float dly = c_fma(rt.x, g2.w, c_fma(s, g2.y, g1.w));
-                                slab_select(g0, dlx, dly, loz, hiz, rt.y, t_max, flat, klow, krow + j);
-                            }
-                        }
-                    }
+                    __syncwarp();
                 }
-                __syncwarp();
             }
         }
         // ---- a5 ground, a7 resolve, a8 shade, a9 store: 4 consecutive pixels per lane ----------
