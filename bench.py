@@ -46,6 +46,8 @@ def parse():
     ap.add_argument("--stage-cap", type=int, default=0, help="GP_OPT_STAGE_CAP override (0 = library default)")
     ap.add_argument("--chunk-worlds", type=int, default=0,
                     help="worlds per gp_render_batch call (0 = as many as keep the planes under 40 GB)")
+    ap.add_argument("--graph", action="store_true",
+                    help="capture each step (pose update + cull + render) in a CUDA graph and time the replays")
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -238,7 +240,21 @@ def run_b200(args):
     for f in range(args.warmup):
         step(f)
     barrier()
-    r.set_option(gp.GP_OPT_TIMING, 1)
+    graphs = None
+    if args.graph:                      # one graph per frame (each reads its own resident pose slice)
+        side = torch.cuda.Stream()
+        graphs = []
+        with torch.cuda.stream(side):
+            for f in range(args.warmup, n_frames):
+                g = torch.cuda.CUDAGraph()
+                with torch.cuda.graph(g, stream=side):
+                    step(f)
+                graphs.append(g)
+        barrier()
+    # per-kernel CUDA events on every 4th step of the timed region (events between all launches would space them out:
+    # +0.8 % on the paper-scale step, +12 % on the small one)
+    timing_every = 4 if args.steps >= 16 else 1
+    r.set_option(gp.GP_OPT_TIMING, 0 if args.graph else timing_every)
     for k in (gp.GP_KERNEL_UPDATE, gp.GP_KERNEL_CULL, gp.GP_KERNEL_RENDER):
         r.kernel_time(k)
     sampler = ClockSampler(local_rank)
@@ -248,13 +264,26 @@ def run_b200(args):
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
     ev0.record()
-    for f in range(args.warmup, n_frames):
-        step(f)
+    if graphs:
+        for g in graphs:
+            g.replay()
+    else:
+        for f in range(args.warmup, n_frames):
+            step(f)
     ev1.record()
     barrier()
     ms = ev0.elapsed_time(ev1)
     clocks = sampler.stop() if rank == 0 else None
     launches = r.launch_count() - launches0
+    if graphs:
+        # replays launch the captured kernels (1 update + cull + render per world chunk and step); per-kernel times
+        # come from a short un-graphed pass after the timed region
+        launches = args.steps * (1 + 2 * len(chunks))
+        r.set_option(gp.GP_OPT_TIMING, 1)
+        for k in (gp.GP_KERNEL_UPDATE, gp.GP_KERNEL_CULL, gp.GP_KERNEL_RENDER):
+            r.kernel_time(k)
+        for f in range(args.warmup, args.warmup + min(10, args.steps)):
+            step(f)
     ktimes = {name: r.kernel_time(k) for name, k in (("update", gp.GP_KERNEL_UPDATE), ("cull", gp.GP_KERNEL_CULL),
                                                        ("render", gp.GP_KERNEL_RENDER))}
     r.set_option(gp.GP_OPT_TIMING, 0)
@@ -332,7 +361,9 @@ def run_b200(args):
         "mpixels_per_s": value * cfg.H * cfg.W / 1e6,
         "clocks": clocks,
         "gpu_launches": int(launches),
-        "kernels_ms_per_step": {k: v[0] / max(1, args.steps) for k, v in ktimes.items()},
+        "kernels_ms_per_step": {k: v[0] / max(1, v[1]) * (len(chunks) if k != "update" else 1) for k, v in ktimes.items()},
+        "kernel_samples": {k: int(v[1]) for k, v in ktimes.items()},
+        "cuda_graph": bool(graphs),
         "roofline": {"bound": "hbm", "kernel": "k_render", "achieved": achieved, "peak": peak, "unit": "GB/s",
                      "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
                      "algorithmic_bytes_per_launch": alg_bytes_launch, "avg_launch_ms": r_avg_ms,

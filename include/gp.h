@@ -44,7 +44,8 @@ enum {
 enum {
     GP_OPT_PATH = 1,        /* GP_PATH_FAST (default) or GP_PATH_BRUTE                        */
     GP_OPT_STATS = 2,       /* 1: count executed ray/primitive tests and listed pairs         */
-    GP_OPT_TIMING = 3,      /* 1: bracket every kernel launch with CUDA events (gp_kernel_time) */
+    GP_OPT_TIMING = 3,      /* n > 0: bracket every n-th launch of each kernel with CUDA events
+                               (gp_kernel_time); 0: off                                         */
     GP_OPT_STAGE_CAP = 4,   /* list entries per view staged in shared memory (default 128, >= 1);
                                longer lists read their tail from global memory                  */
     GP_OPT_STRIP_PX = 5,    /* target pixels per warp strip of the render pass; 0 = automatic   */
@@ -176,8 +177,8 @@ int gp_render_batch_host(gp_ctx *ctx, const float *h_pose, int world_begin, int 
  * pairs that survived the cull.  Either pointer may be NULL. */
 int gp_stats(gp_ctx *ctx, uint64_t *executed_tests, uint64_t *listed_pairs);
 
-/* With GP_OPT_TIMING = 1 every launch of the library is bracketed by CUDA events on the launch
- * stream.  Returns the summed device time (milliseconds) and the number of launches of `kernel`
+/* With GP_OPT_TIMING = n > 0 every n-th launch of each kernel is bracketed by CUDA events on the launch
+ * stream (n > 1 keeps the event records from spacing out back-to-back launches).  Returns the summed device time (milliseconds) and the number of launches of `kernel`
  * recorded since the last call for that kernel, then forgets them.  Synchronises the device. */
 int gp_kernel_time(gp_ctx *ctx, int kernel, double *total_ms, uint64_t *launches);
 

@@ -34,6 +34,7 @@ struct gp_ctx {
     std::vector<Timed> timed;                                    // GP_OPT_TIMING records
     std::vector<cudaEvent_t> ev_pool;
     uint64_t launches = 0;
+    unsigned timing_seq[4] = {0, 0, 0, 0};
     size_t render_smem_set = 0;
     // gp_render_batch_host staging
     float *d_pose = nullptr;
@@ -52,7 +53,9 @@ static int cuda_fail(cudaError_t e, const char *where) {
 // Brackets one kernel launch with events when GP_OPT_TIMING is on.
 struct LaunchTimer {
     gp_ctx *c; cudaStream_t s; bool on; gp_ctx::Timed t{};
-    LaunchTimer(gp_ctx *c_, int kernel, cudaStream_t s_) : c(c_), s(s_), on(c_->opt_timing != 0) {
+    LaunchTimer(gp_ctx *c_, int kernel, cudaStream_t s_) : c(c_), s(s_), on(false) {
+        if (c->opt_timing <= 0) return;
+        on = (c->timing_seq[kernel & 3]++ % (unsigned)c->opt_timing) == 0;     // every opt_timing-th launch of this kernel
         if (!on) return;
         t.kernel = kernel;
         cudaEvent_t *e[2] = {&t.a, &t.b};
@@ -140,7 +143,10 @@ extern "C" int gp_set_option(gp_ctx *c, int key, int value) {
         case GP_OPT_STATS:
             c->opt_stats = value ? 1 : 0; return GP_OK;
         case GP_OPT_TIMING:
-            c->opt_timing = value ? 1 : 0; return GP_OK;
+            if (value < 0) return GP_ERR_ARG;
+            c->opt_timing = value;
+            for (unsigned &q : c->timing_seq) q = 0;
+            return GP_OK;
         case GP_OPT_STAGE_CAP:
             if (value < 1) return GP_ERR_ARG;
             c->opt_stage_cap = value; return GP_OK;
