@@ -100,7 +100,10 @@ constexpr int kCullWarps = 8;          // views per CTA (one warp per view), all
 
 // Grid: one CTA per (world, group of kCullWarps views of that world).  The world's records (first 32 bytes of each:
 // centre, half extents, heading) are staged in shared memory once per CTA and shared by its views.
-__global__ void __launch_bounds__(kCullWarps * 32, 3)
+#ifndef GP_CULL_MIN_CTAS
+#define GP_CULL_MIN_CTAS 4
+#endif
+__global__ void __launch_bounds__(kCullWarps * 32, GP_CULL_MIN_CTAS)
 k_cull(SceneConst sc, const gp_prim *__restrict__ prims, const float2 *__restrict__ pitch,
        int world_begin, int groups_per_world, int H, int W, float th, float tv,
        ViewHdr *__restrict__ hdr, EntryGeo *__restrict__ geo, EntryAux *__restrict__ aux, int cap,
@@ -238,9 +241,9 @@ k_cull(SceneConst sc, const gp_prim *__restrict__ prims, const float2 *__restric
                     const int d = c | bit;
                     const float Xa = cX[c], Xb = cX[d];
                     if ((Xa < near) == (Xb < near)) continue;
-                    const float t = (near - Xa) / (Xb - Xa);
+                    const float t = (near - Xa) * rcp_fast(Xb - Xa);       // |Xb - Xa| > 0 here; error covered by E below
                     const float Yi = cY[c] + t * (cY[d] - cY[c]), Zi = cZ[c] + t * (cZ[d] - cZ[c]);
-                    bound_point(b, near, Yi, Zi, E);
+                    bound_point(b, near, Yi, Zi, E + 1e-6f * (fabsf(cY[d] - cY[c]) + fabsf(cZ[d] - cZ[c])));
                     qYmin = fminf(qYmin, Yi); qYmax = fmaxf(qYmax, Yi);
                     qZmin = fminf(qZmin, Zi); qZmax = fmaxf(qZmax, Zi);
                 }
