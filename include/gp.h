@@ -127,6 +127,15 @@ int gp_scene_upload(gp_ctx *ctx, const gp_scene_desc *desc, const gp_prim *h_age
  * aligned.  No host transfer. */
 int gp_agents_update(gp_ctx *ctx, const float *d_pose, void *stream);
 
+/* Replace static primitives from device memory.  d_prims: DEVICE [Wn][n] gp_prim records (16-byte aligned) that
+ * overwrite static slots [q_begin, q_begin + n) of every world (primitives A + q_begin ...), verbatim; their
+ * shading tables are refreshed.  Fields are NOT validated (cls is masked to 0..7; a shape other than
+ * GP_SHAPE_SPHERE is a box).  A scene uploaded without spheres keeps rendering without the sphere code path, so
+ * spheres introduced here are ignored unless the uploaded scene already held one.  With agents_per_world = 1
+ * this gives the paper's one-world-per-ego layout: the ego is the agent, everything else static
+ * slots refreshed per step without a host transfer. */
+int gp_statics_update(gp_ctx *ctx, const gp_prim *d_prims, int n, int q_begin, void *stream);
+
 /* Static map from polylines, on the device (C1p; "lane polylines ... thin planar strips",
  * :331 "road geometry, encoded as polyline segments").  d_points: DEVICE [Wn][n_lines][pts_per_line][2] fp32
  * (x, y), 8-byte aligned.  Segment s of line l of world w overwrites static primitive number

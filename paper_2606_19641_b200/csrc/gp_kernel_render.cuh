@@ -381,7 +381,7 @@ k_render(SceneConst sc, RenderArgs ra) {
     extern __shared__ __align__(16) unsigned char smem[];
     const int view = blockIdx.x;
     const int H = ra.H, W = ra.W, SR = ra.SR;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
 
     // ---- shared memory carve-up ---------------------------------------------------------------
     uint64_t *bar = reinterpret_cast<uint64_t *>(smem);

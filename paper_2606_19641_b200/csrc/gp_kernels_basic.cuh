@@ -45,6 +45,18 @@ __global__ void k_agents_update(SceneConst sc, const float4 *__restrict__ pose, 
     write_meta(q, &meta[w * sc.P + a], sc);
 }
 
+// a0 for static slots: records copied from device memory + their shading table.
+__global__ void k_statics_update(SceneConst sc, const gp_prim *__restrict__ src, int n, int q_begin,
+                                 gp_prim *__restrict__ prims, PrimMeta *__restrict__ meta) {
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= (size_t)sc.Wn * n) return;
+    const size_t w = i / n, q = i % n;
+    const gp_prim p = src[i];
+    const size_t k = w * sc.P + sc.A + q_begin + q;
+    prims[k] = p;
+    write_meta(p, &meta[k], sc);
+}
+
 // C1p: one thread per polyline segment -> flat quad record + its shading table.
 __global__ void k_polyline_quads(SceneConst sc, const float2 *__restrict__ pts, int n_lines, int pts_per_line,
                                  float half_width, float z, int cls, int q_begin, gp_prim *__restrict__ prims,

@@ -233,6 +233,19 @@ extern "C" int gp_agents_update(gp_ctx *c, const float *d_pose, void *stream_) {
     return GP_OK;
 }
 
+extern "C" int gp_statics_update(gp_ctx *c, const gp_prim *d_prims, int n, int q_begin, void *stream_) {
+    if (!c || !d_prims || n < 1) return GP_ERR_ARG;
+    if (!c->have_scene) return GP_ERR_STATE;
+    if (!aligned16(d_prims)) return GP_ERR_ALIGN;
+    if (q_begin < 0 || (long long)q_begin + n > c->sc.Q) return GP_ERR_RANGE;
+    const size_t total = (size_t)c->sc.Wn * n;
+    k_statics_update<<<(unsigned)((total + 255) / 256), 256, 0, static_cast<cudaStream_t>(stream_)>>>(
+        c->sc, d_prims, n, q_begin, c->d_prims, c->d_meta);
+    c->launches += 1;
+    CK(cudaGetLastError());
+    return GP_OK;
+}
+
 extern "C" int gp_statics_from_polylines(gp_ctx *c, const float *d_points, int n_lines, int pts_per_line,
                                          float half_width, float z, int cls, int q_begin, void *stream_) {
     if (!c || !d_points) return GP_ERR_ARG;

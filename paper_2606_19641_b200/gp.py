@@ -21,7 +21,7 @@ GP_PATH_FAST, GP_PATH_BRUTE = 0, 1
 
 EXPORTS = ("gp_create", "gp_destroy", "gp_set_option", "gp_scene_upload", "gp_agents_update",
            "gp_cameras_set", "gp_render_batch", "gp_render_batch_host", "gp_stats", "gp_kernel_time",
-           "gp_launch_count", "gp_camera_rig_set", "gp_statics_from_polylines",
+           "gp_launch_count", "gp_camera_rig_set", "gp_statics_from_polylines", "gp_statics_update",
            "gp_error_string")
 
 
@@ -71,6 +71,7 @@ def lib():
         L.gp_kernel_time.argtypes = [vp, ci, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_uint64)]
         L.gp_launch_count.argtypes = [vp, ctypes.POINTER(ctypes.c_uint64)]
         L.gp_camera_rig_set.argtypes = [vp, ci, vp]
+        L.gp_statics_update.argtypes = [vp, vp, ci, ci, vp]
         L.gp_statics_from_polylines.argtypes = [vp, vp, ci, ci, cf, cf, ci, ci, vp]
         L.gp_error_string.argtypes = [ci]
         L.gp_error_string.restype = ctypes.c_char_p
@@ -144,6 +145,11 @@ class Renderer:
     def cameras_set(self, d_pitch_cs=None):
         """d_pitch_cs: CUDA float32 tensor [Wn][A][2] = (cos p, sin p), or None for pitch 0."""
         _check(lib().gp_cameras_set(self._h, _dptr(d_pitch_cs), _stream()))
+
+    def statics_update(self, d_prims, q_begin=0):
+        """d_prims: CUDA uint8 tensor [Wn][n][48] of gp_prim records replacing static slots q_begin .. of every world."""
+        assert d_prims.dim() == 3 and d_prims.shape[2] == 48 and d_prims.is_contiguous()
+        _check(lib().gp_statics_update(self._h, _dptr(d_prims), int(d_prims.shape[1]), int(q_begin), _stream()))
 
     def statics_from_polylines(self, d_points, half_width=0.075, z=0.01, cls=2, q_begin=0):
         """d_points: CUDA float32 tensor [Wn][n_lines][pts_per_line][2]; one flat quad per segment replaces the

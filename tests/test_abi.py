@@ -61,6 +61,7 @@ def test_null_arguments_are_rejected_without_a_gpu(libgp):
     assert libgp.gp_render_batch(None, 0, 1, 1, 8, 8, 1.0, None, None, None, None, None) == gp.GP_ERR_ARG
     assert libgp.gp_stats(None, None, None) == gp.GP_ERR_ARG
     assert libgp.gp_camera_rig_set(None, 1, None) == gp.GP_ERR_ARG
+    assert libgp.gp_statics_update(None, None, 1, 0, None) == gp.GP_ERR_ARG
     assert libgp.gp_statics_from_polylines(None, None, 1, 2, 0.1, 0.0, 2, 0, None) == gp.GP_ERR_ARG
 
 
