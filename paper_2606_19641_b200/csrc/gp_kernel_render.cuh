@@ -22,6 +22,7 @@ struct RenderArgs {
     float th, tv;
     int SR, log2LC;                 // rows per strip; lanes per row of the test tile (LC = 1 << log2LC)
     int log2W;                      // valid when NG > 0 (W a power of two)
+    int ngr; uint32_t magicW;       // NG == 0: groups per whole strip when SR*W % 128 == 0 and W % 4 == 0 (else 0); ceil(2^32 / W)
     uint8_t *o_cls; int32_t *o_inst; float *o_depth; uint8_t *o_rgb;
     unsigned long long *stats;
 };
@@ -645,6 +646,15 @@ k_render(SceneConst sc, RenderArgs ra) {
                     const int row = row0 + ((lane * 4 + it * 128) >> ra.log2W);
                     resolve_quad(s_row[row].w, s_bg, kq ? kq + it * 128 : nullptr, wtab, pc + it * 128,
                                  pi + it * 128, pd + it * 128, pr ? pr + it * 128 : nullptr, HW);
+                }
+            } else if (ra.ngr > 0 && row1 - row0 + 1 == SR) {
+                // W % 4 == 0 and the strip is a whole number of 128-pixel groups (e.g. 96 x 4, 192 x 2, 112 x 8):
+                // no row straddling, no ragged tail; the row of a pixel by a multiply-high with ceil(2^32 / W)
+                for (int it = 0; it < ra.ngr; ++it) {
+                    const int off = it * 128;
+                    const int row = row0 + (int)__umulhi((unsigned)(lane * 4 + off), ra.magicW);
+                    resolve_quad(s_row[row].w, s_bg, kq ? kq + off : nullptr, wtab, pc + off, pi + off, pd + off,
+                                 pr ? pr + off : nullptr, HW);
                 }
             } else {
                 // any W: the strip is SR*W consecutive pixels (a multiple of 4, start 4-aligned); a lane's

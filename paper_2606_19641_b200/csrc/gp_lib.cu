@@ -365,14 +365,31 @@ static int render_device(gp_ctx *c, int world_begin, int n_worlds, int H, int W,
     int SR = align;
     while (SR < 16 && SR * 2 * W <= strip_px) SR *= 2;
     if ((W & (W - 1)) && c->opt_strip_px <= 0) {
-        // width not a power of two: a strip is resolved in groups of 128 consecutive pixels, so prefer the
-        // strip height (multiple of `align`, up to ~1024 pixels, >= 8 strips per view) whose last group is fullest
-        double best = -1.0;
-        for (int cand = align; cand <= 16; cand += align) {
-            const int px = cand * W;
-            if (cand > align && (px > 1024 || (H + cand - 1) / cand < 8)) break;
-            const double eff = (double)px / (double)(((px + 127) / 128) * 128);
-            if (eff > best + 0.02) { best = eff; SR = cand; }
+        // Width not a power of two: a strip is resolved in groups of 128 consecutive pixels, so the strip height
+        // (a multiple of `align`) decides how full the last group is.  Measured on B200: strips of more
+        // than ~640 pixels cost occupancy (8-byte key per pixel per warp), fewer than 4 strips per warp cost balance;
+        // so take the fullest last group among heights giving <= 640 pixels and enough strips, nearest to 512 pixels
+        // on ties, and go up to 1024 pixels only if nothing smaller fills 85 % (210 x 126: 4 rows = 840 pixels).
+        // Heights above 2 are multiples of 4: the test tile walks a strip 4 rows at a time.
+        const int need = (long long)H * W <= 64 * 64 ? 8 : 16;
+        for (int limit = 640; limit <= 1024; limit += 384) {
+            double best = -1.0;
+            for (int cand = align; cand <= 16; cand += align) {
+                const int px = cand * W;
+                if (cand > align && (px > limit || (H + cand - 1) / cand < need)) break;
+                if (cand > 2 && (cand & 3)) continue;
+                const double eff = (double)px / (double)(((px + 127) / 128) * 128);
+                if (eff > best) best = eff;
+            }
+            int best_px = -1;
+            for (int cand = align; cand <= 16; cand += align) {
+                const int px = cand * W;
+                if (cand > align && (px > limit || (H + cand - 1) / cand < need)) break;
+                if (cand > 2 && (cand & 3)) continue;
+                const double eff = (double)px / (double)(((px + 127) / 128) * 128);
+                if (eff >= best - 0.02 && (best_px < 0 || abs(px - 512) < abs(best_px - 512))) { best_px = px; SR = cand; }
+            }
+            if (best >= 0.85) break;
         }
     }
     ra.SR = SR;
@@ -384,6 +401,8 @@ static int render_device(gp_ctx *c, int world_begin, int n_worlds, int H, int W,
     ra.log2W = log2W;
     int ng = 0;                                                    // unrolled resolve: NG groups of 128 pixels
     if ((1 << log2W) == W && H % SR == 0 && (SR * W == 128 || SR * W == 256 || SR * W == 512)) ng = SR * W / 128;
+    ra.ngr = (ng == 0 && (W & 3) == 0 && (SR * W) % 128 == 0) ? SR * W / 128 : 0;
+    ra.magicW = (uint32_t)((0x100000000ull + (unsigned)W - 1) / (unsigned)W);
     const int n_strips = (H + SR - 1) / SR;
     // warps per CTA (= per view): 4; 2 for images of up to 64 x 64 pixels, where twice as many (shorter-lived) CTAs
     // per SM hide the per-view prologue better (32 x 32: 0.230 -> 0.174 ms, 64 x 64: 0.457 -> 0.384 ms; measured slower
