@@ -41,6 +41,7 @@ def parse():
     ap.add_argument("--workload", default="paper", choices=list(gs.CONFIGS))
     ap.add_argument("--worlds", type=int, default=0, help="override the number of worlds (debug)")
     ap.add_argument("--res", type=int, default=0, help="override H = W (resolution sweep)")
+    ap.add_argument("--hw", type=int, nargs=2, default=None, metavar=("H", "W"), help="override the image size")
     ap.add_argument("--strip-px", type=int, default=0, help="GP_OPT_STRIP_PX override (0 = library default)")
     ap.add_argument("--gather", type=int, default=-1, help="GP_OPT_GATHER override (-1 = library default)")
     ap.add_argument("--stage-cap", type=int, default=0, help="GP_OPT_STAGE_CAP override (0 = library default)")
@@ -116,6 +117,8 @@ def workload_cfg(args):
         cfg = cfg.replace(n_worlds=args.worlds)
     if args.res:
         cfg = cfg.replace(H=args.res, W=args.res)
+    if args.hw:
+        cfg = cfg.replace(H=args.hw[0], W=args.hw[1])
     return cfg
 
 
@@ -343,7 +346,7 @@ def run_b200(args):
     achieved = alg_bytes_launch / (r_avg_ms * 1e-3) / 1e9
     traffic = None
     tpath = os.path.join(ROOT, "profiles", "r01_traffic.txt")      # from the committed ncu --set full capture
-    if os.path.exists(tpath) and not args.worlds and not args.res:
+    if os.path.exists(tpath) and not args.worlds and not args.res and not args.hw:
         for line in open(tpath):
             part = line.split()
             if len(part) == 2 and part[0] == cfg.name:
