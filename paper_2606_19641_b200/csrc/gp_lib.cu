@@ -413,6 +413,7 @@ static int render_device(gp_ctx *c, int world_begin, int n_worlds, int H, int W,
     // (the same list over fewer pixels) or crowded worlds; entry-by-entry is ~1 % faster on the store-bound cases.
     int gather = c->opt_gather;
     if (gather < 0) gather = ((long long)H * W <= 96 * 96 || sc.P >= 400) ? 1 : 0;
+    if (sc.P > 65535) gather = 0;                                  // the per-warp overlap list holds 16-bit entry indices
     const size_t smem = 48 + (size_t)ra.scap * 64 + (size_t)H * 16 + (size_t)((W + 3) & ~3) * 4 +
                         (gather ? (size_t)nwarps * kOverlapCap * sizeof(uint16_t) : 0) + (size_t)nwarps * SR * W * 8;
     if (smem > 227 * 1024) return GP_ERR_ARG;
