@@ -39,6 +39,28 @@ __device__ __forceinline__ void bound_point(PixBounds &b, float X, float Y, floa
     b.vmin = fminf(b.vmin, v - dv); b.vmax = fmaxf(b.vmax, v + dv);
 }
 
+// Does the box (camera frame: centre (Xc, Yc, Zc), half-edge vectors (Xx, Yx, Zx), (Xy, Yy, Zy), (Xz, 0, Zz)) reach
+// into the tip cuboid [0, near] x [-gdY, gdY] x [-gdZ, gdZ] of the view pyramid?  Conservative separating-axis test
+// over the camera's Y and Z axes (the caller established the overlap in X) and the three box axes.  Out of line: it
+// runs only for primitives that straddle the near clip plane, and must not cost the main path registers.
+__device__ __noinline__ bool box_meets_tip(float Xc, float Yc, float Zc, float Xx, float Xy, float Xz, float Yx, float Yy,
+                                           float Zx, float Zy, float Zz, float near, float gdY, float gdZ, float E) {
+    const float Yr = fabsf(Yx) + fabsf(Yy), Zr = fabsf(Zx) + fabsf(Zy) + fabsf(Zz);
+    if (!(fabsf(Yc) - Yr < gdY && fabsf(Zc) - Zr < gdZ)) return false;
+    const float ex[3] = {Xx, Xy, Xz}, ey[3] = {Yx, Yy, 0.0f}, ez[3] = {Zx, Zy, Zz};   // X, Y, Z parts of the half-edge vectors
+#pragma unroll
+    for (int m = 0; m < 3; ++m) {
+        const float ax = ex[m], ay = ey[m], az = ez[m];
+        const float dist = fabsf(ax * (Xc - 0.5f * near) + ay * Yc + az * Zc);
+        float r = 0.0f;
+#pragma unroll
+        for (int q = 0; q < 3; ++q) r += fabsf(ax * ex[q] + ay * ey[q] + az * ez[q]);
+        const float rt = fabsf(ax) * (0.5f * near + E) + fabsf(ay) * gdY + fabsf(az) * gdZ;
+        if (dist > (r + rt) * 1.0001f + 1e-9f) return false;
+    }
+    return true;
+}
+
 // Camera of the view (contract C2) and everything of C5 that depends only on (view, primitive).
 struct CullCam { float ox, oy, oz, fx, fy, rx, ry, ux, uy, cp, sp; };
 struct CullPrim {
@@ -248,10 +270,16 @@ k_cull(SceneConst sc, const gp_prim *__restrict__ prims, const float2 *__restric
                     qZmin = fminf(qZmin, Zi); qZmax = fmaxf(qZmax, Zi);
                 }
             }
-            // the part of the box with 0 < X < near projects outside the bound above only if the
-            // cross-section comes close to the optical centre: then give up and take the whole image
-            const float gd = kNearGuard + E;
-            if (qYmin <= gd && qYmax >= -gd && qZmin <= gd && qZmax >= -gd) full = true;
+            // The part of the box with 0 < X < near is not covered by the bound above.  A point of it is inside
+            // the image only if |Y| < th X < th near and |Z| < tv near, i.e. only if the box reaches into the tip
+            // of the view pyramid; then give up and take the whole image.  Two conservative tests of that: the
+            // cross-section at X = near, and the camera-frame bounding intervals of the box, both against the tip
+            // widened to at least kNearGuard (the tip is large for extreme fields of view: tv near = 10 m at a
+            // 4096 x 4 image).
+            const float gdY = fmaxf(kNearGuard, 1.01f * th * near) + E, gdZ = fmaxf(kNearGuard, 1.01f * tv * near) + E;
+            if (qYmin <= gdY && qYmax >= -gdY && qZmin <= gdZ && qZmax >= -gdZ) full = true;
+            if (!full && fabsf(Yc) - (fabsf(Yx) + fabsf(Yy)) < gdY && fabsf(Zc) - (fabsf(Zx) + fabsf(Zy) + fabsf(Zz)) < gdZ)
+                full = box_meets_tip(Xc, Yc, Zc, Xx, Xy, Xz, Yx, Yy, Zx, Zy, Zz, near, gdY, gdZ, E);   // rare
         }
         int c0, c1, r0, r1;
         if (full) { c0 = 0; c1 = W - 1; r0 = 0; r1 = H - 1; }
