@@ -123,7 +123,7 @@ constexpr int kCullWarps = 8;          // views per CTA (one warp per view), all
 // Grid: one CTA per (world, group of kCullWarps views of that world).  The world's records (first 32 bytes of each:
 // centre, half extents, heading) are staged in shared memory once per CTA and shared by its views.
 #ifndef GP_CULL_MIN_CTAS
-#define GP_CULL_MIN_CTAS 4
+#define GP_CULL_MIN_CTAS 3
 #endif
 __global__ void __launch_bounds__(kCullWarps * 32, GP_CULL_MIN_CTAS)
 k_cull(SceneConst sc, const gp_prim *__restrict__ prims, const float2 *__restrict__ pitch,
