@@ -65,7 +65,7 @@ def peaks():
 
 class ClockSampler:
     """nvidia-smi clocks and throttle reasons DURING the timed region."""
-    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+    Q = ("clocks.sm,clocks.max.sm,clocks.mem,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
          "clocks_event_reasons.sw_power_cap")
 
@@ -95,20 +95,20 @@ class ClockSampler:
             self.proc.wait(timeout=5)
         except subprocess.TimeoutExpired:
             self.proc.kill()
-        sm, mx, reasons = [], [], set()
+        sm, mx, mem, reasons = [], [], [], set()
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
         for r in self.rows:
             if len(r) < 7:
                 continue
             try:
-                sm.append(float(r[0])); mx.append(float(r[1]))
+                sm.append(float(r[0])); mx.append(float(r[1])); mem.append(float(r[2]))
             except ValueError:
                 continue
             for n, v in zip(names, r[3:7]):
                 if v.lower().startswith("active"):
                     reasons.add(n)
         return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
-                "samples": len(sm), "reasons": sorted(reasons)}
+                "mem_mhz": statistics.median(mem) if mem else None, "samples": len(sm), "reasons": sorted(reasons)}
 
 
 def workload_cfg(args):
@@ -382,7 +382,10 @@ def run_b200(args):
         per_core_s = 0.09 * (cfg.H * cfg.W * cfg.prims) / (128 * 128 * 264)
         n_views = int(min(cfg.views, max(threads, round(40.0 * threads / per_core_s))))
         sec = oracle_sample(cfg, n_views, threads)
+        n1 = max(1, min(cfg.views, int(round(1.5 / per_core_s))))
+        sec1 = oracle_sample(cfg, n1, 1)
         out["cpu_baseline"] = {"value": n_views / sec, "unit": UNIT, "cores": threads, "kind": "oracle",
+                               "one_core": {"value": n1 / sec1, "unit": UNIT, "sample": "%d views, 1 thread, %.1f s" % (n1, sec1)},
                                "sample": "%d views of the workload (frame 0), all-primitive fp32 oracle (oracle/gp_oracle.c), %d threads, %.1f s"
                                          % (n_views, threads, sec)}
     print(json.dumps(out))
