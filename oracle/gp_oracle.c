@@ -25,7 +25,9 @@
  *                      the fp32 renderer against the contract itself being wrong.
  *
  * Pins (tests/test_oracle_pins.py, -m "not gpu"): closed forms CF1-CF6, brute force vs the
- * fp64 face enumeration, invariants I1-I9.  Nothing here is
+ * fp64 face enumeration, invariants I1-I9, the edge rule U10; tests/test_oracle_pitch_pins.py:
+ * the pitched camera basis of C2 (f, r, u) on primitives under pitch, from angle-built fp64
+ * geometry that does not pass through orc_shadow_view.  Nothing here is
  * "parity unpinned"; none of the pins come from the paper, which prints no value for this
  * path.
  *

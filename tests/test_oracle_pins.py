@@ -415,3 +415,21 @@ def test_primitive_beats_the_ground_at_equal_depth():
     assert (r["depth"][covered] == g["depth"][covered]).all()
     assert (r["t2"][covered] == r["depth"][covered]).all()          # the ground is the tied runner-up
     assert (r["inst"][covered] == 9).all()
+
+
+def test_u10_ray_through_a_vertical_box_edge_takes_the_x_face():
+    # Reading U10: on an exact edge (lo_x == lo_y == t_n) the entry face is x.  A 1 x 1 image has s = v = 0
+    # exactly, so the single ray is the optical axis; a box with yaw 45 deg (cos == sin in fp32) and hx == hy
+    # centred on the axis presents its vertical edge to it, and the two slab entries are the same fp32 number
+    # by symmetry.  Camera heading -x: the two candidate faces are +x_local (n.L = (0.48 + 0.36) c) and
+    # -y_local (n.L = (0.48 - 0.36) c), c = cos 45 deg — different shades, so the choice is visible.
+    c = np.float32(math.sqrt(0.5))
+    D, h = 20.0, 1.0
+    box = make_prim(-D, 0.0, 1.6, h, h, 1.0, c, c, inst=4)
+    r = oracle.render_view(stack(ego_at_origin(-1, 0), box), 0, 1, 1)
+    assert r["cls"][0, 0] == VEH and r["inst"][0, 0] == 4
+    assert abs(r["depth"][0, 0] - (D - h * math.sqrt(2.0))) < 1e-5 * D
+    x_face = shade(PAL[VEH], (0.48 + 0.36) * float(c))
+    y_face = shade(PAL[VEH], (0.48 - 0.36) * float(c))
+    assert x_face != y_face
+    assert tuple(int(v) for v in r["rgb"][:, 0, 0]) == x_face
