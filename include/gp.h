@@ -49,9 +49,14 @@ enum {
     GP_OPT_STAGE_CAP = 4,   /* list entries per view staged in shared memory (default 128, >= 1);
                                longer lists read their tail from global memory                  */
     GP_OPT_STRIP_PX = 5,    /* target pixels per warp strip of the render pass; 0 = automatic   */
-    GP_OPT_GATHER = 6       /* how a strip works off its list: 1 gather the overlapping entries first, one lane
+    GP_OPT_GATHER = 6,      /* how a strip works off its list: 1 gather the overlapping entries first, one lane
                                per (flat quad, row); 0 entry by entry; -1 (default) chosen from the image size
                                and the primitives per world                                        */
+    GP_OPT_SPHERES = 7      /* are records with shape == GP_SHAPE_SPHERE drawn?  -1 (default) automatic: yes iff the
+                               uploaded scene held a sphere or gp_statics_update has run since the upload (its
+                               records are device memory the host never inspects); 1 yes; 0 no: sphere records
+                               are skipped by every path alike (the render pass then runs without the sphere
+                               branch, which costs the box-only case a few per cent)                 */
 };
 enum {                      /* kernel ids of gp_kernel_time                                   */
     GP_KERNEL_UPDATE = 0,   /* a0 pose update + shading table                                 */
@@ -130,8 +135,8 @@ int gp_agents_update(gp_ctx *ctx, const float *d_pose, void *stream);
 /* Replace static primitives from device memory.  d_prims: DEVICE [Wn][n] gp_prim records (16-byte aligned) that
  * overwrite static slots [q_begin, q_begin + n) of every world (primitives A + q_begin ...), verbatim; their
  * shading tables are refreshed.  Fields are NOT validated (cls is masked to 0..7; a shape other than
- * GP_SHAPE_SPHERE is a box).  A scene uploaded without spheres keeps rendering without the sphere code path, so
- * spheres introduced here are ignored unless the uploaded scene already held one.  With agents_per_world = 1
+ * GP_SHAPE_SPHERE is a box).  Spheres introduced here are drawn: after this call the render pass runs with its
+ * sphere branch (see GP_OPT_SPHERES to declare that no sphere will ever be written).  With agents_per_world = 1
  * this gives the paper's one-world-per-ego layout: the ego is the agent, everything else static
  * slots refreshed per step without a host transfer. */
 int gp_statics_update(gp_ctx *ctx, const gp_prim *d_prims, int n, int q_begin, void *stream);
@@ -165,8 +170,9 @@ int gp_camera_rig_set(gp_ctx *ctx, int n_cams, const gp_camera *h_rig);
  *   d_instance [n][H][W]    int32   the winning primitive's inst; -1 for ground and sky
  *   d_depth    [n][H][W]    float   planar depth of the nearest hit; 0 for sky
  *   d_rgb      [n][3][H][W] uint8   shaded colour, planar; NULL skips the plane
- * 1 <= H, W <= 4096.  The fast path needs W >= 4 and (H * W) % 4 == 0 (e.g. 210 x 126, 434 x 252);
- * other sizes take the brute-force path.
+ * 1 <= H, W <= 4096.  The fast path needs W >= 4 and (H * W) % 4 == 0 (e.g. 210 x 126, 434 x 252) and one
+ * warp's strip of the image in shared memory (fails only for widths near 4096 that are not a multiple of 4);
+ * other sizes take the brute-force path, with identical results.
  * May grow library-owned scratch on first use of a larger (n_worlds, H, W): warm up before timing. */
 int gp_render_batch(gp_ctx *ctx, int world_begin, int n_worlds, int agents, int H, int W,
                     float fov_rad, uint8_t *d_class, int32_t *d_instance, float *d_depth,
@@ -174,9 +180,10 @@ int gp_render_batch(gp_ctx *ctx, int world_begin, int n_worlds, int agents, int 
 
 /* End-to-end variant with HOST buffers: copies h_pose (HOST [Wn][A][4], may be NULL = keep poses) to the
  * device, updates the agents, renders worlds [world_begin, world_begin+n_worlds) in chunks through
- * library-owned device staging and copies the four planes (same layouts as above; h_rgb may be NULL)
- * back to the HOST buffers.  Synchronises `stream` before returning.  Pinned host memory is faster
- * but not required. */
+ * library-owned device staging and copies the planes (same layouts as above) back to the HOST buffers.
+ * Any of the four plane pointers may be NULL (not all): that plane is not copied back — the path is bound by
+ * the host link (PCIe), so a consumer that needs e.g. only depth moves a third of the bytes.  Synchronises
+ * `stream` before returning.  Pinned host memory is faster but not required. */
 int gp_render_batch_host(gp_ctx *ctx, const float *h_pose, int world_begin, int n_worlds, int agents,
                          int H, int W, float fov_rad, uint8_t *h_class, int32_t *h_instance,
                          float *h_depth, uint8_t *h_rgb, void *stream);

@@ -191,7 +191,7 @@ k_cull(SceneConst sc, const gp_prim *__restrict__ prims, const float2 *__restric
         for (int kb = k0; kb < k1; kb += 32) {
             const int k = kb + lane;
             bool pass = false;
-            if (k < k1 && k != a) {
+            if (k < k1 && k != a && (sc.spheres || !s_sphere[k - k0])) {
                 const float4 p0 = s_p0[k - k0];                                           // cx cy cz hx
                 const float dx = p0.x - cam.ox, dy = p0.y - cam.oy, dz = p0.z - cam.oz;
                 const float R = s_R[k - k0];

@@ -211,38 +211,48 @@ __device__ __forceinline__ EntryRec load_entry(const StripBatchCtx &c, int eb) {
     return r;
 }
 
-// Conservative column interval [ja, jb] of a flat entry on the row with table entry rt (not contract
-// arithmetic: plain fp32 + slack): the plane depth t is fixed per row, so the footprint is one interval.
-__device__ __forceinline__ void flat_interval(const EntryRec &E, const float4 &rt, const StripBatchCtx &c, int &ja, int &jb) {
-    const float4 &g0 = E.g0, &g1 = E.g1, &g2 = E.g2;
-    const int c0 = (int)(E.ax.z & 0xffff), c1 = (int)(E.ax.z >> 16);
-    ja = 1; jb = 0;
+// Conservative column interval [ja, jb] of a flat entry on one image row (not contract arithmetic: plain fp32 +
+// slack): the plane depth t is fixed per row, so the footprint of the quad on that row is one interval.
+// flat_prepare: the part that depends on the entry only; flat_row: one row.
+struct FlatBound { float mx, my, hxs, hys, col_scale, halfW; };
+__device__ __forceinline__ FlatBound flat_prepare(const float4 &g0, const float4 &g1, int W, float th) {
+    FlatBound fb;
     // centre -ol and half extents h in the ray-origin frame, recovered from a = -h - ol, b = h - ol
-    const float mx = 0.5f * (g0.x + g0.y), my = 0.5f * (g0.z + g0.w), mz = 0.5f * (g1.x + g1.y);
+    fb.mx = 0.5f * (g0.x + g0.y); fb.my = 0.5f * (g0.z + g0.w);
+    const float mz = 0.5f * (g1.x + g1.y);
     const float ex_ = 0.5f * (g0.y - g0.x), ey_ = 0.5f * (g0.w - g0.z);
-    const float dl_ = 2e-5f * (fabsf(mx) + fabsf(my) + fabsf(mz) + ex_ + ey_) + 1e-6f;
-    const float hxs = ex_ + dl_, hys = ey_ + dl_;
+    const float dl_ = 2e-5f * (fabsf(fb.mx) + fabsf(fb.my) + fabsf(mz) + ex_ + ey_) + 1e-6f;
+    fb.hxs = ex_ + dl_; fb.hys = ey_ + dl_;
+    fb.col_scale = 0.5f * (float)W / th; fb.halfW = 0.5f * (float)W;
+    return fb;
+}
+__device__ __forceinline__ void flat_row(const FlatBound &fb, const float4 &g1, const float4 &g2, const float4 &rt,
+                                         float t_max, int W, int c0, int c1, int &ja, int &jb) {
+    ja = 1; jb = 0;
     const float t = g1.x * rt.z;                     // plane depth on this row
-    if (!(t > 0.0f && t <= c.t_max * 1.00001f)) return;
-    const float X0 = fmaf(t, fmaf(rt.x, g2.z, g1.z), -mx), X1 = t * g2.x;
-    const float Y0 = fmaf(t, fmaf(rt.x, g2.w, g1.w), -my), Y1 = t * g2.y;
+    if (!(t > 0.0f && t <= t_max * 1.00001f)) return;
+    const float X0 = fmaf(t, fmaf(rt.x, g2.z, g1.z), -fb.mx), X1 = t * g2.x;
+    const float Y0 = fmaf(t, fmaf(rt.x, g2.w, g1.w), -fb.my), Y1 = t * g2.y;
     float slo = -3.0e38f, shi = 3.0e38f;
     bool ok = true;
     if (fabsf(X1) > 1e-12f) {
-        const float r = flat_rcp(X1), a = (-hxs - X0) * r, b = (hxs - X0) * r;
+        const float r = flat_rcp(X1), a = (-fb.hxs - X0) * r, b = (fb.hxs - X0) * r;
         slo = fmaxf(slo, fminf(a, b)); shi = fminf(shi, fmaxf(a, b));
-    } else ok = fabsf(X0) <= hxs;
+    } else ok = fabsf(X0) <= fb.hxs;
     if (fabsf(Y1) > 1e-12f) {
-        const float r = flat_rcp(Y1), a = (-hys - Y0) * r, b = (hys - Y0) * r;
+        const float r = flat_rcp(Y1), a = (-fb.hys - Y0) * r, b = (fb.hys - Y0) * r;
         slo = fmaxf(slo, fminf(a, b)); shi = fminf(shi, fmaxf(a, b));
-    } else ok = ok && fabsf(Y0) <= hys;
+    } else ok = ok && fabsf(Y0) <= fb.hys;
     if (!(ok && slo <= shi)) return;
     // column of s: (s/th + 1) W/2 - 0.5, widened by 0.02 px + relative slack
-    const float col_scale = 0.5f * (float)c.W / c.th;
-    const float xa = fmaf(slo, col_scale, 0.5f * (float)c.W - 0.52f) - 1e-5f * fabsf(slo * col_scale);
-    const float xb = fmaf(shi, col_scale, 0.5f * (float)c.W - 0.48f) + 1e-5f * fabsf(shi * col_scale);
+    const float xa = fmaf(slo, fb.col_scale, fb.halfW - 0.52f) - 1e-5f * fabsf(slo * fb.col_scale);
+    const float xb = fmaf(shi, fb.col_scale, fb.halfW - 0.48f) + 1e-5f * fabsf(shi * fb.col_scale);
     ja = max(c0, (int)ceilf(fmaxf(xa, -1.0f)));
-    jb = min(c1, (int)floorf(fminf(xb, (float)c.W)));
+    jb = min(c1, (int)floorf(fminf(xb, (float)W)));
+}
+__device__ __forceinline__ void flat_interval(const EntryRec &E, const float4 &rt, const StripBatchCtx &c, int &ja, int &jb) {
+    const FlatBound fb = flat_prepare(E.g0, E.g1, c.W, c.th);
+    flat_row(fb, E.g1, E.g2, rt, c.t_max, c.W, (int)(E.ax.z & 0xffff), (int)(E.ax.z >> 16), ja, jb);
 }
 
 // The gathered entries of one strip: olist[0 .. nfl) flat quads, olist[kOverlapCap - nbx .. kOverlapCap) boxes and
@@ -559,41 +569,14 @@ k_render(SceneConst sc, RenderArgs ra) {
                         // Wide flat primitive: per row, the plane depth t is fixed, so the footprint is one
                         // column interval.  Bound it conservatively (plain fp32 + slack) and run the exact
                         // test only inside it: a thin diagonal marking costs ~its length, not its bbox area.
-                        // (not contract arithmetic: centre -ol and half extents h in the ray-origin frame, recovered from
-                        // a = -h - ol, b = h - ol)
-                        const float mx = 0.5f * (g0.x + g0.y), my = 0.5f * (g0.z + g0.w), mz = 0.5f * (g1.x + g1.y);
-                        const float ex_ = 0.5f * (g0.y - g0.x), ey_ = 0.5f * (g0.w - g0.z);
-                        const float dl_ = 2e-5f * (fabsf(mx) + fabsf(my) + fabsf(mz) + ex_ + ey_) + 1e-6f;
-                        const float hxs = ex_ + dl_, hys = ey_ + dl_;
-                        const float col_scale = 0.5f * (float)W / ra.th;
+                        const FlatBound fb = flat_prepare(g0, g1, W, ra.th);       // conservative bound, not contract arithmetic
                         for (int rb = r0; rb <= r1; rb += LR) {
                             const int i = rb + li;
                             int ja = 1, jb = 0;                                  // empty
                             float4 rt = make_float4(0.f, 0.f, 0.f, 0.f);
                             if (i <= r1) {
                                 rt = s_row[i];
-                                const float t = g1.x * rt.z;                     // plane depth on this row
-                                if (t > 0.0f && t <= t_max * 1.00001f) {
-                                    const float X0 = fmaf(t, fmaf(rt.x, g2.z, g1.z), -mx), X1 = t * g2.x;
-                                    const float Y0 = fmaf(t, fmaf(rt.x, g2.w, g1.w), -my), Y1 = t * g2.y;
-                                    float slo = -3.0e38f, shi = 3.0e38f;
-                                    bool ok = true;
-                                    if (fabsf(X1) > 1e-12f) {
-                                        const float r = flat_rcp(X1), a = (-hxs - X0) * r, b = (hxs - X0) * r;
-                                        slo = fmaxf(slo, fminf(a, b)); shi = fminf(shi, fmaxf(a, b));
-                                    } else ok = fabsf(X0) <= hxs;
-                                    if (fabsf(Y1) > 1e-12f) {
-                                        const float r = flat_rcp(Y1), a = (-hys - Y0) * r, b = (hys - Y0) * r;
-                                        slo = fmaxf(slo, fminf(a, b)); shi = fminf(shi, fmaxf(a, b));
-                                    } else ok = ok && fabsf(Y0) <= hys;
-                                    if (ok && slo <= shi) {
-                                        // column of s: (s/th + 1) W/2 - 0.5, widened by 0.02 px + relative slack
-                                        const float xa = fmaf(slo, col_scale, 0.5f * (float)W - 0.52f) - 1e-5f * fabsf(slo * col_scale);
-                                        const float xb = fmaf(shi, col_scale, 0.5f * (float)W - 0.48f) + 1e-5f * fabsf(shi * col_scale);
-                                        ja = max(c0, (int)ceilf(fmaxf(xa, -1.0f)));
-                                        jb = min(c1, (int)floorf(fminf(xb, (float)W)));
-                                    }
-                                }
+                                flat_row(fb, g1, g2, rt, t_max, W, c0, c1, ja, jb);
                             }
                             float loz, hiz;
                             slab_z(g1, rt, loz, hiz);

@@ -125,6 +125,7 @@ k_render_brute(SceneConst sc, const gp_prim *__restrict__ prims, const float2 *_
             if (k == a) continue;
             const gp_prim p = wp[k];
             if (p.shape == GP_SHAPE_SPHERE) {                       // C5s
+                if (!sc.spheres) continue;
                 const float dx = c_fma(v, ux, c_fma(s, rx, fx)), dy = c_fma(v, uy, c_fma(s, ry, fy));
                 const float tn = sphere_entry(c_sub(ox, p.cx), c_sub(oy, p.cy), c_sub(oz, p.cz), c_mul(p.hx, p.hx), dx, dy, dz);
                 if (!(tn > 0.0f && tn <= sc.t_max)) continue;
@@ -168,7 +169,7 @@ k_render_brute(SceneConst sc, const gp_prim *__restrict__ prims, const float2 *_
         else if (best_k == -1) { c = 1; id = -1; dep = best_t; s8 = shade_scale(c_max(sc.Lz, 0.0f), sc.ambient); }
         else {
             const gp_prim p = wp[best_k];
-            c = p.cls; id = p.inst; dep = best_t;
+            c = p.cls & 7; id = p.inst; dep = best_t;             // unvalidated device records: same mask as the resolve table
             const float qx = c_fma(p.sin_yaw, sc.Ly, c_mul(p.cos_yaw, sc.Lx));
             const float qy = c_fma(p.cos_yaw, sc.Ly, -c_mul(p.sin_yaw, sc.Lx));
             const float qm = best_m == 0 ? qx : best_m == 1 ? qy : sc.Lz;

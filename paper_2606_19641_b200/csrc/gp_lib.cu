@@ -19,7 +19,8 @@ using namespace gp;
 
 struct gp_ctx {
     int device = -1;
-    bool have_scene = false, has_spheres = false;
+    bool have_scene = false, has_spheres = false;     // has_spheres: the uploaded records held a sphere
+    bool statics_touched = false;                     // gp_statics_update ran since the upload (may have added spheres)
     SceneConst sc{};
     gp_prim *d_prims = nullptr;
     PrimMeta *d_meta = nullptr;
@@ -29,7 +30,7 @@ struct gp_ctx {
     ViewHdr *d_hdr = nullptr; EntryGeo *d_geo = nullptr; EntryAux *d_aux = nullptr;
     size_t scratch_views = 0; int scratch_cap = 0;
     unsigned long long *d_stats = nullptr;
-    int opt_path = GP_PATH_FAST, opt_stats = 0, opt_timing = 0, opt_stage_cap = GP_STAGE_CAP, opt_strip_px = 0, opt_gather = -1;
+    int opt_path = GP_PATH_FAST, opt_stats = 0, opt_timing = 0, opt_stage_cap = GP_STAGE_CAP, opt_strip_px = 0, opt_gather = -1, opt_spheres = -1;
     struct Timed { int kernel; cudaEvent_t a, b; };
     std::vector<Timed> timed;                                    // GP_OPT_TIMING records
     std::vector<cudaEvent_t> ev_pool;
@@ -50,13 +51,21 @@ static int cuda_fail(cudaError_t e, const char *where) {
 }
 #define CK(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cuda_fail(e_, #call); } while (0)
 
-// Brackets one kernel launch with events when GP_OPT_TIMING is on.
+// Brackets one kernel launch with events when GP_OPT_TIMING is on.  At most kMaxTimed records are kept.
+constexpr size_t kMaxTimed = 4096;
 struct LaunchTimer {
     gp_ctx *c; cudaStream_t s; bool on; gp_ctx::Timed t{};
     LaunchTimer(gp_ctx *c_, int kernel, cudaStream_t s_) : c(c_), s(s_), on(false) {
         if (c->opt_timing <= 0) return;
+        cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;              // no event records inside a graph capture
+        if (cudaStreamIsCapturing(s, &cap) != cudaSuccess) { cudaGetLastError(); return; }
+        if (cap != cudaStreamCaptureStatusNone) return;
         on = (c->timing_seq[kernel & 3]++ % (unsigned)c->opt_timing) == 0;     // every opt_timing-th launch of this kernel
         if (!on) return;
+        if (c->timed.size() >= kMaxTimed) {                                     // never polled: recycle the oldest record
+            c->ev_pool.push_back(c->timed.front().a); c->ev_pool.push_back(c->timed.front().b);
+            c->timed.erase(c->timed.begin());
+        }
         t.kernel = kernel;
         cudaEvent_t *e[2] = {&t.a, &t.b};
         for (auto p : e) {
@@ -69,6 +78,18 @@ struct LaunchTimer {
 };
 
 static bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+// Every ABI entry runs on the context's device, whatever device the calling thread had current, and leaves the
+// caller's current device as it found it.
+struct DeviceGuard {
+    int prev = -1; bool ok = true;
+    explicit DeviceGuard(const gp_ctx *c) {
+        if (cudaGetDevice(&prev) != cudaSuccess) { prev = -1; cudaGetLastError(); }
+        if (prev != c->device) ok = cudaSetDevice(c->device) == cudaSuccess; else prev = -1;
+    }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+#define GP_ON_DEVICE(c) DeviceGuard guard_(c); if (!guard_.ok) return cuda_fail(cudaGetLastError(), "cudaSetDevice")
 
 extern "C" const char *gp_error_string(int code) {
     switch (code) {
@@ -117,7 +138,8 @@ static void free_scene(gp_ctx *c) {
 
 extern "C" int gp_destroy(gp_ctx *c) {
     if (!c) return GP_ERR_ARG;
-    cudaSetDevice(c->device);
+    {
+    GP_ON_DEVICE(c);
     cudaDeviceSynchronize();
     free_scene(c);
     for (int i = 0; i < 2; ++i) {
@@ -130,6 +152,7 @@ extern "C" int gp_destroy(gp_ctx *c) {
     if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
     if (c->h_stage) cudaFreeHost(c->h_stage);
     cudaFree(c->d_stats);
+    }
     delete c;
     return GP_OK;
 }
@@ -153,6 +176,9 @@ extern "C" int gp_set_option(gp_ctx *c, int key, int value) {
         case GP_OPT_GATHER:
             if (value < -1 || value > 1) return GP_ERR_ARG;
             c->opt_gather = value; return GP_OK;
+        case GP_OPT_SPHERES:
+            if (value < -1 || value > 1) return GP_ERR_ARG;
+            c->opt_spheres = value; return GP_OK;
         case GP_OPT_STRIP_PX:
             if (value < 0 || value > 4096) return GP_ERR_ARG;
             c->opt_strip_px = value; return GP_OK;
@@ -183,7 +209,7 @@ extern "C" int gp_scene_upload(gp_ctx *c, const gp_scene_desc *d, const gp_prim 
     for (size_t i = 0; i < Wn * A; ++i) spheres |= h_agents[i].shape == GP_SHAPE_SPHERE;
     for (size_t i = 0; i < Wn * Q; ++i) spheres |= h_quads[i].shape == GP_SHAPE_SPHERE;
     cudaStream_t stream = static_cast<cudaStream_t>(stream_);
-    CK(cudaSetDevice(c->device));
+    GP_ON_DEVICE(c);
     CK(cudaDeviceSynchronize());            // earlier work may still read the old scene
     free_scene(c);
     if (c->h_stage_bytes < n * sizeof(gp_prim)) {
@@ -215,6 +241,7 @@ extern "C" int gp_scene_upload(gp_ctx *c, const gp_scene_desc *d, const gp_prim 
     CK(cudaGetLastError());
     c->have_scene = true;
     c->has_spheres = spheres;
+    c->statics_touched = false;
     return GP_OK;
 }
 
@@ -222,6 +249,7 @@ extern "C" int gp_agents_update(gp_ctx *c, const float *d_pose, void *stream_) {
     if (!c || !d_pose) return GP_ERR_ARG;
     if (!c->have_scene) return GP_ERR_STATE;
     if (!aligned16(d_pose)) return GP_ERR_ALIGN;
+    GP_ON_DEVICE(c);
     const size_t n = (size_t)c->sc.Wn * c->sc.A;
     {
         LaunchTimer lt(c, GP_KERNEL_UPDATE, static_cast<cudaStream_t>(stream_));
@@ -238,6 +266,8 @@ extern "C" int gp_statics_update(gp_ctx *c, const gp_prim *d_prims, int n, int q
     if (!c->have_scene) return GP_ERR_STATE;
     if (!aligned16(d_prims)) return GP_ERR_ALIGN;
     if (q_begin < 0 || (long long)q_begin + n > c->sc.Q) return GP_ERR_RANGE;
+    GP_ON_DEVICE(c);
+    c->statics_touched = true;      // the records are device memory the host never sees: they may hold spheres
     const size_t total = (size_t)c->sc.Wn * n;
     k_statics_update<<<(unsigned)((total + 255) / 256), 256, 0, static_cast<cudaStream_t>(stream_)>>>(
         c->sc, d_prims, n, q_begin, c->d_prims, c->d_meta);
@@ -254,6 +284,7 @@ extern "C" int gp_statics_from_polylines(gp_ctx *c, const float *d_points, int n
     if (reinterpret_cast<uintptr_t>(d_points) & 7u) return GP_ERR_ALIGN;
     const long long per_world = (long long)n_lines * (pts_per_line - 1);
     if (q_begin < 0 || q_begin + per_world > c->sc.Q) return GP_ERR_RANGE;
+    GP_ON_DEVICE(c);
     const size_t n = (size_t)c->sc.Wn * (size_t)per_world;
     k_polyline_quads<<<(unsigned)((n + 255) / 256), 256, 0, static_cast<cudaStream_t>(stream_)>>>(
         c->sc, reinterpret_cast<const float2 *>(d_points), n_lines, pts_per_line, half_width, z, cls, q_begin,
@@ -266,6 +297,7 @@ extern "C" int gp_statics_from_polylines(gp_ctx *c, const float *d_points, int n
 extern "C" int gp_cameras_set(gp_ctx *c, const float *d_pitch_cs, void *stream_) {
     if (!c) return GP_ERR_ARG;
     if (!c->have_scene) return GP_ERR_STATE;
+    GP_ON_DEVICE(c);
     const size_t n = (size_t)c->sc.Wn * c->sc.A;
     cudaStream_t stream = static_cast<cudaStream_t>(stream_);
     if (d_pitch_cs) {
@@ -317,46 +349,10 @@ static int check_render_args(gp_ctx *c, int world_begin, int n_worlds, int agent
     return GP_OK;
 }
 
-// Enqueue cull + render (or the brute-force kernel) for a world range into DEVICE planes.
-static int render_device(gp_ctx *c, int world_begin, int n_worlds, int H, int W, float fov_rad,
-                         uint8_t *d_class, int32_t *d_instance, float *d_depth, uint8_t *d_rgb,
-                         cudaStream_t stream) {
-    const SceneConst &sc = c->sc;
-    const float th = (float)tan(0.5 * (double)fov_rad);          // C2, host side
-    const float tv = th * ((float)H / (float)W);
-    const size_t views = (size_t)n_worlds * sc.A * sc.C;
-    if (views > 0x7fffffffull) return GP_ERR_ARG;
-    unsigned long long *stats = c->opt_stats ? c->d_stats : nullptr;
-    if (stats) CK(cudaMemsetAsync(stats, 0, 2 * sizeof(unsigned long long), stream));
-
-    // fast path: every view (H*W pixels) must start 16-byte aligned in the 32-bit planes
-    if (c->opt_path == GP_PATH_BRUTE || W < 4 || (((long long)H * W) & 3)) {
-        const int HW = H * W;
-        dim3 grid((unsigned)views, (unsigned)std::min((HW + 255) / 256, 65535));
-        {
-            LaunchTimer lt(c, GP_KERNEL_BRUTE, stream);
-            k_render_brute<<<grid, 256, 0, stream>>>(sc, c->d_prims, c->d_pitch, world_begin, H, W, th, tv,
-                                                      d_class, d_instance, d_depth, d_rgb);
-        }
-        c->launches += 1;
-        CK(cudaGetLastError());
-        return GP_OK;
-    }
-    int rc = ensure_scratch(c, views);
-    if (rc != GP_OK) return rc;
-    {
-        LaunchTimer lt(c, GP_KERNEL_CULL, stream);
-        const int gpw = (sc.A * sc.C + kCullWarps - 1) / kCullWarps;   // CTAs per world
-        k_cull<<<(unsigned)((size_t)n_worlds * gpw), kCullWarps * 32, 0, stream>>>(
-            sc, c->d_prims, c->d_pitch, world_begin, gpw, H, W, th, tv,
-                                                    c->d_hdr, c->d_geo, c->d_aux, c->scratch_cap, stats);
-    }
-    c->launches += 1;
-    CK(cudaGetLastError());
-
-    RenderArgs ra;
-    ra.hdr = c->d_hdr; ra.geo = c->d_geo; ra.aux = c->d_aux; ra.meta = c->d_meta;
-    ra.cap = c->scratch_cap; ra.scap = std::min(c->scratch_cap, c->opt_stage_cap); ra.world_begin = world_begin; ra.H = H; ra.W = W; ra.th = th; ra.tv = tv;
+// Launch shape of the render pass for an H x W image (host logic; all thresholds measured on B200).
+struct RenderPlan { int SR, log2LC, log2W, ng, ngr, nwarps, gather, scap; uint32_t magicW; size_t smem; };
+static bool plan_render(const gp_ctx *c, const SceneConst &sc, int H, int W, RenderPlan &pl) {
+    pl.scap = std::min(sc.P, c->opt_stage_cap);
     // rows per strip (power of two): ~512 pixels, fewer for small images so that a view still has
     // >= 16 strips to spread over its warps (a strip's entries are processed serially by one warp)
     int strip_px = c->opt_strip_px;
@@ -392,31 +388,91 @@ static int render_device(gp_ctx *c, int world_begin, int n_worlds, int H, int W,
             if (best >= 0.85) break;
         }
     }
-    ra.SR = SR;
+    pl.SR = SR;
     const int LR = SR >= 4 ? 4 : SR >= 2 ? 2 : 1;              // rows of the test tile (power of two)
-    ra.log2LC = LR == 4 ? 3 : LR == 2 ? 4 : 5;
-    ra.o_cls = d_class; ra.o_inst = d_instance; ra.o_depth = d_depth; ra.o_rgb = d_rgb; ra.stats = stats;
+    pl.log2LC = LR == 4 ? 3 : LR == 2 ? 4 : 5;
     int log2W = 0;
     while ((1 << log2W) < W) ++log2W;
-    ra.log2W = log2W;
+    pl.log2W = log2W;
     int ng = 0;                                                    // unrolled resolve: NG groups of 128 pixels
     if ((1 << log2W) == W && H % SR == 0 && (SR * W == 128 || SR * W == 256 || SR * W == 512)) ng = SR * W / 128;
-    ra.ngr = (ng == 0 && (W & 3) == 0 && (SR * W) % 128 == 0) ? SR * W / 128 : 0;
-    ra.magicW = (uint32_t)((0x100000000ull + (unsigned)W - 1) / (unsigned)W);
+    pl.ngr = (ng == 0 && (W & 3) == 0 && (SR * W) % 128 == 0) ? SR * W / 128 : 0;
+    pl.magicW = (uint32_t)((0x100000000ull + (unsigned)W - 1) / (unsigned)W);
     const int n_strips = (H + SR - 1) / SR;
     // warps per CTA (= per view): 4; 2 for images of up to 64 x 64 pixels, where twice as many (shorter-lived) CTAs
     // per SM hide the per-view prologue better (32 x 32: 0.230 -> 0.174 ms, 64 x 64: 0.457 -> 0.384 ms; measured slower
     // from 128 x 128 up)
     const int max_warps = (long long)H * W <= 64 * 64 ? (GP_RENDER_WARPS < 2 ? GP_RENDER_WARPS : 2) : GP_RENDER_WARPS;
-    const int nwarps = n_strips < max_warps ? n_strips : max_warps;
+    int nwarps = n_strips < max_warps ? n_strips : max_warps;
     // List handling (measured on B200): gathering pays when many entries meet a strip — small images
     // (the same list over fewer pixels) or crowded worlds; entry-by-entry is ~1 % faster on the store-bound cases.
     int gather = c->opt_gather;
     if (gather < 0) gather = ((long long)H * W <= 96 * 96 || sc.P >= 400) ? 1 : 0;
     if (sc.P > 65535) gather = 0;                                  // the per-warp overlap list holds 16-bit entry indices
-    const size_t smem = 48 + (size_t)ra.scap * 64 + (size_t)H * 16 + (size_t)((W + 3) & ~3) * 4 +
-                        (gather ? (size_t)nwarps * kOverlapCap * sizeof(uint16_t) : 0) + (size_t)nwarps * SR * W * 8;
-    if (smem > 227 * 1024) return GP_ERR_ARG;
+    // shared memory: list stage + row / column tables + per-warp overlap list and key buffer; very wide images
+    // get fewer warps per view, and the caller takes the brute-force path if even one warp does not fit
+    size_t smem;
+    for (;; --nwarps) {
+        smem = 48 + (size_t)pl.scap * 64 + (size_t)H * 16 + (size_t)((W + 3) & ~3) * 4 +
+               (gather ? (size_t)nwarps * kOverlapCap * sizeof(uint16_t) : 0) + (size_t)nwarps * SR * W * 8;
+        if (smem <= 227 * 1024 || nwarps == 1) break;
+    }
+    pl.ng = ng; pl.nwarps = nwarps; pl.gather = gather; pl.smem = smem;
+    return smem <= 227 * 1024;
+}
+
+// Enqueue cull + render (or the brute-force kernel) for a world range into DEVICE planes.
+static int render_device(gp_ctx *c, int world_begin, int n_worlds, int H, int W, float fov_rad,
+                         uint8_t *d_class, int32_t *d_instance, float *d_depth, uint8_t *d_rgb,
+                         cudaStream_t stream) {
+    // Spheres are drawn iff the uploaded scene held one or gp_statics_update has run since (its records are device
+    // memory the host never sees), unless GP_OPT_SPHERES says otherwise; when off, sphere records are skipped by
+    // every path alike (cull and brute force), so the result stays well defined.
+    const bool spheres = c->opt_spheres >= 0 ? c->opt_spheres != 0 : (c->has_spheres || c->statics_touched);
+    SceneConst sc = c->sc;
+    sc.spheres = spheres ? 1 : 0;
+    const float th = (float)tan(0.5 * (double)fov_rad);          // C2, host side
+    const float tv = th * ((float)H / (float)W);
+    const size_t views = (size_t)n_worlds * sc.A * sc.C;
+    if (views > 0x7fffffffull) return GP_ERR_ARG;
+    unsigned long long *stats = c->opt_stats ? c->d_stats : nullptr;
+    if (stats) CK(cudaMemsetAsync(stats, 0, 2 * sizeof(unsigned long long), stream));
+
+    // fast path: every view (H*W pixels) must start 16-byte aligned in the 32-bit planes, and one warp's strip
+    // must fit shared memory (it does not for e.g. 4096 x 4094: odd widths force 2- or 4-row strips)
+    RenderPlan pl{};
+    const bool fast_ok = W >= 4 && !(((long long)H * W) & 3) && plan_render(c, sc, H, W, pl);
+    if (c->opt_path == GP_PATH_BRUTE || !fast_ok) {
+        const int HW = H * W;
+        dim3 grid((unsigned)views, (unsigned)std::min((HW + 255) / 256, 65535));
+        {
+            LaunchTimer lt(c, GP_KERNEL_BRUTE, stream);
+            k_render_brute<<<grid, 256, 0, stream>>>(sc, c->d_prims, c->d_pitch, world_begin, H, W, th, tv,
+                                                      d_class, d_instance, d_depth, d_rgb);
+        }
+        c->launches += 1;
+        CK(cudaGetLastError());
+        return GP_OK;
+    }
+    int rc = ensure_scratch(c, views);
+    if (rc != GP_OK) return rc;
+    {
+        LaunchTimer lt(c, GP_KERNEL_CULL, stream);
+        const int gpw = (sc.A * sc.C + kCullWarps - 1) / kCullWarps;   // CTAs per world
+        k_cull<<<(unsigned)((size_t)n_worlds * gpw), kCullWarps * 32, 0, stream>>>(
+            sc, c->d_prims, c->d_pitch, world_begin, gpw, H, W, th, tv,
+                                                    c->d_hdr, c->d_geo, c->d_aux, c->scratch_cap, stats);
+    }
+    c->launches += 1;
+    CK(cudaGetLastError());
+
+    RenderArgs ra;
+    ra.hdr = c->d_hdr; ra.geo = c->d_geo; ra.aux = c->d_aux; ra.meta = c->d_meta;
+    ra.cap = c->scratch_cap; ra.scap = pl.scap; ra.world_begin = world_begin; ra.H = H; ra.W = W; ra.th = th; ra.tv = tv;
+    ra.SR = pl.SR; ra.log2LC = pl.log2LC; ra.log2W = pl.log2W; ra.ngr = pl.ngr; ra.magicW = pl.magicW;
+    ra.o_cls = d_class; ra.o_inst = d_instance; ra.o_depth = d_depth; ra.o_rgb = d_rgb; ra.stats = stats;
+    const int ng = pl.ng, nwarps = pl.nwarps, gather = pl.gather;
+    const size_t smem = pl.smem;
     typedef void (*RenderFn)(SceneConst, RenderArgs);
 #define GP_FNS(ST, SP, GA) {k_render<ST, 0, SP, GA>, k_render<ST, 1, SP, GA>, k_render<ST, 2, SP, GA>, k_render<ST, 4, SP, GA>}
     static const RenderFn fns[2][2][2][4] = {      // [gather][spheres][stats][ng index]
@@ -433,7 +489,7 @@ static int render_device(gp_ctx *c, int world_begin, int n_worlds, int H, int W,
     }
     {
         LaunchTimer lt(c, GP_KERNEL_RENDER, stream);
-        const RenderFn fn = fns[gather][c->has_spheres ? 1 : 0][stats ? 1 : 0][ng == 4 ? 3 : ng];
+        const RenderFn fn = fns[gather][spheres ? 1 : 0][stats ? 1 : 0][ng == 4 ? 3 : ng];
         fn<<<dim3((unsigned)views), dim3(nwarps * 32), smem, stream>>>(sc, ra);
     }
     c->launches += 1;
@@ -448,6 +504,7 @@ extern "C" int gp_render_batch(gp_ctx *c, int world_begin, int n_worlds, int age
     if (rc != GP_OK) return rc;
     if (!d_class || !d_instance || !d_depth) return GP_ERR_ARG;
     if (!aligned16(d_class) || !aligned16(d_instance) || !aligned16(d_depth) || !aligned16(d_rgb)) return GP_ERR_ALIGN;
+    GP_ON_DEVICE(c);
     return render_device(c, world_begin, n_worlds, H, W, fov_rad, d_class, d_instance, d_depth, d_rgb,
                          static_cast<cudaStream_t>(stream_));
 }
@@ -457,11 +514,12 @@ extern "C" int gp_render_batch_host(gp_ctx *c, const float *h_pose, int world_be
                                     float *h_depth, uint8_t *h_rgb, void *stream_) {
     int rc = check_render_args(c, world_begin, n_worlds, agents, H, W, fov_rad);
     if (rc != GP_OK) return rc;
-    if (!h_class || !h_instance || !h_depth) return GP_ERR_ARG;
+    if (!h_class && !h_instance && !h_depth && !h_rgb) return GP_ERR_ARG;
+    GP_ON_DEVICE(c);
     cudaStream_t stream = static_cast<cudaStream_t>(stream_);
     const SceneConst &sc = c->sc;
     const size_t HW = (size_t)H * W, A = (size_t)sc.A * sc.C;      // A: views per world here
-    const size_t bpv = HW * (h_rgb ? 12 : 9);                     // output bytes per view
+    const size_t bpv = HW * 12;                                   // staged bytes per view (all planes are rendered)
     // chunk: <= 512 MiB of planes per staging buffer, at least one world
     size_t wc = (512ull << 20) / (bpv * A);
     if (wc < 1) wc = 1;
@@ -494,16 +552,16 @@ extern "C" int gp_render_batch_host(gp_ctx *c, const float *h_pose, int world_be
         unsigned char *base = c->d_out[buf];
         uint8_t *dc = base; int32_t *di = reinterpret_cast<int32_t *>(base + plane);
         float *dd = reinterpret_cast<float *>(base + plane * 5);
-        uint8_t *dr = h_rgb ? base + plane * 9 : nullptr;
+        uint8_t *dr = h_rgb ? base + plane * 9 : nullptr;           // the rgb plane is not even rendered when unwanted
         CK(cudaStreamWaitEvent(stream, c->ev_copy[buf], 0));      // staging buffer free again
         rc = render_device(c, world_begin + (int)w0, (int)nw, H, W, fov_rad, dc, di, dd, dr, stream);
         if (rc != GP_OK) return rc;
         CK(cudaEventRecord(c->ev_render[buf], stream));
         CK(cudaStreamWaitEvent(c->copy_stream, c->ev_render[buf], 0));
         const size_t v0 = w0 * A;
-        CK(cudaMemcpyAsync(h_class + v0 * HW, dc, nv * HW, cudaMemcpyDeviceToHost, c->copy_stream));
-        CK(cudaMemcpyAsync(h_instance + v0 * HW, di, nv * HW * 4, cudaMemcpyDeviceToHost, c->copy_stream));
-        CK(cudaMemcpyAsync(h_depth + v0 * HW, dd, nv * HW * 4, cudaMemcpyDeviceToHost, c->copy_stream));
+        if (h_class) CK(cudaMemcpyAsync(h_class + v0 * HW, dc, nv * HW, cudaMemcpyDeviceToHost, c->copy_stream));
+        if (h_instance) CK(cudaMemcpyAsync(h_instance + v0 * HW, di, nv * HW * 4, cudaMemcpyDeviceToHost, c->copy_stream));
+        if (h_depth) CK(cudaMemcpyAsync(h_depth + v0 * HW, dd, nv * HW * 4, cudaMemcpyDeviceToHost, c->copy_stream));
         if (h_rgb) CK(cudaMemcpyAsync(h_rgb + v0 * HW * 3, dr, nv * HW * 3, cudaMemcpyDeviceToHost, c->copy_stream));
         CK(cudaEventRecord(c->ev_copy[buf], c->copy_stream));
     }
@@ -515,6 +573,7 @@ extern "C" int gp_render_batch_host(gp_ctx *c, const float *h_pose, int world_be
 extern "C" int gp_stats(gp_ctx *c, uint64_t *executed_tests, uint64_t *listed_pairs) {
     if (!c) return GP_ERR_ARG;
     unsigned long long h[2];
+    GP_ON_DEVICE(c);
     CK(cudaDeviceSynchronize());
     CK(cudaMemcpy(h, c->d_stats, sizeof h, cudaMemcpyDeviceToHost));
     if (executed_tests) *executed_tests = h[0];
@@ -524,6 +583,7 @@ extern "C" int gp_stats(gp_ctx *c, uint64_t *executed_tests, uint64_t *listed_pa
 
 extern "C" int gp_kernel_time(gp_ctx *c, int kernel, double *total_ms, uint64_t *launches) {
     if (!c || !total_ms || !launches) return GP_ERR_ARG;
+    GP_ON_DEVICE(c);
     CK(cudaDeviceSynchronize());
     double ms = 0.0; uint64_t n = 0;
     std::vector<gp_ctx::Timed> keep;

@@ -15,7 +15,7 @@ LIB_PATH = os.path.join(_HERE, "libgp.so")
 
 GP_OK, GP_ERR_ARG, GP_ERR_ALIGN, GP_ERR_STATE, GP_ERR_RANGE, GP_ERR_CUDA, GP_ERR_ARCH, GP_ERR_NOMEM = \
     0, -1, -2, -3, -4, -5, -6, -7
-GP_OPT_PATH, GP_OPT_STATS, GP_OPT_TIMING, GP_OPT_STAGE_CAP, GP_OPT_STRIP_PX, GP_OPT_GATHER = 1, 2, 3, 4, 5, 6
+GP_OPT_PATH, GP_OPT_STATS, GP_OPT_TIMING, GP_OPT_STAGE_CAP, GP_OPT_STRIP_PX, GP_OPT_GATHER, GP_OPT_SPHERES = 1, 2, 3, 4, 5, 6, 7
 GP_KERNEL_UPDATE, GP_KERNEL_CULL, GP_KERNEL_RENDER, GP_KERNEL_BRUTE = 0, 1, 2, 3
 GP_PATH_FAST, GP_PATH_BRUTE = 0, 1
 
@@ -86,9 +86,9 @@ def _check(rc):
         raise GpError(rc, lib().gp_error_string(rc).decode())
 
 
-def _stream():
+def _stream(device):
     import torch
-    return ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)
+    return ctypes.c_void_p(torch.cuda.current_stream(device).cuda_stream)
 
 
 def _dptr(t):
@@ -135,28 +135,28 @@ class Renderer:
             for ch in range(3):
                 d.palette[c][ch] = int(palette[c][ch])
         _check(lib().gp_scene_upload(self._h, ctypes.byref(d), agents.ctypes.data,
-                                     quads.ctypes.data if Q else None, _stream()))
+                                     quads.ctypes.data if Q else None, _stream(self.device)))
         self.desc = d
 
     def agents_update(self, d_pose):
         """d_pose: CUDA float32 tensor [Wn][A][4] = (cx, cy, cos yaw, sin yaw)."""
-        _check(lib().gp_agents_update(self._h, _dptr(d_pose), _stream()))
+        _check(lib().gp_agents_update(self._h, _dptr(d_pose), _stream(self.device)))
 
     def cameras_set(self, d_pitch_cs=None):
         """d_pitch_cs: CUDA float32 tensor [Wn][A][2] = (cos p, sin p), or None for pitch 0."""
-        _check(lib().gp_cameras_set(self._h, _dptr(d_pitch_cs), _stream()))
+        _check(lib().gp_cameras_set(self._h, _dptr(d_pitch_cs), _stream(self.device)))
 
     def statics_update(self, d_prims, q_begin=0):
         """d_prims: CUDA uint8 tensor [Wn][n][48] of gp_prim records replacing static slots q_begin .. of every world."""
         assert d_prims.dim() == 3 and d_prims.shape[2] == 48 and d_prims.is_contiguous()
-        _check(lib().gp_statics_update(self._h, _dptr(d_prims), int(d_prims.shape[1]), int(q_begin), _stream()))
+        _check(lib().gp_statics_update(self._h, _dptr(d_prims), int(d_prims.shape[1]), int(q_begin), _stream(self.device)))
 
     def statics_from_polylines(self, d_points, half_width=0.075, z=0.01, cls=2, q_begin=0):
         """d_points: CUDA float32 tensor [Wn][n_lines][pts_per_line][2]; one flat quad per segment replaces the
         static primitives q_begin .. of every world."""
         assert d_points.dim() == 4 and d_points.shape[3] == 2 and d_points.is_contiguous()
         _check(lib().gp_statics_from_polylines(self._h, _dptr(d_points), int(d_points.shape[1]), int(d_points.shape[2]),
-                                               float(half_width), float(z), int(cls), int(q_begin), _stream()))
+                                               float(half_width), float(z), int(cls), int(q_begin), _stream(self.device)))
 
     def camera_rig_set(self, rig):
         """rig: array-like [C][>=3] = (cos yaw offset, sin yaw offset, mount) per camera of every agent."""
@@ -172,7 +172,7 @@ class Renderer:
         n = n_worlds * agents * cameras."""
         _check(lib().gp_render_batch(self._h, int(world_begin), int(n_worlds), int(self.desc.agents_per_world),
                                      int(H), int(W), float(fov_rad), _dptr(d_class), _dptr(d_instance),
-                                     _dptr(d_depth), _dptr(d_rgb), _stream()))
+                                     _dptr(d_depth), _dptr(d_rgb), _stream(self.device)))
 
     def render_batch_host(self, h_pose, world_begin, n_worlds, H, W, fov_rad, h_class, h_instance, h_depth,
                           h_rgb=None):
@@ -183,7 +183,7 @@ class Renderer:
             return ctypes.c_void_p(x.ctypes.data if isinstance(x, np.ndarray) else x.data_ptr())
         _check(lib().gp_render_batch_host(self._h, hp(h_pose), int(world_begin), int(n_worlds),
                                           int(self.desc.agents_per_world), int(H), int(W), float(fov_rad),
-                                          hp(h_class), hp(h_instance), hp(h_depth), hp(h_rgb), _stream()))
+                                          hp(h_class), hp(h_instance), hp(h_depth), hp(h_rgb), _stream(self.device)))
 
     def stats(self):
         a, b = ctypes.c_uint64(), ctypes.c_uint64()
