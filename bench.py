@@ -45,6 +45,9 @@ def parse():
     ap.add_argument("--strip-px", type=int, default=0, help="GP_OPT_STRIP_PX override (0 = library default)")
     ap.add_argument("--gather", type=int, default=-1, help="GP_OPT_GATHER override (-1 = library default)")
     ap.add_argument("--stage-cap", type=int, default=0, help="GP_OPT_STAGE_CAP override (0 = library default)")
+    ap.add_argument("--variant", type=int, default=-1, help="GP_OPT_VARIANT: 0 ray strips, 1 raster tiles, -1 library default")
+    ap.add_argument("--tile-px", type=int, default=0, help="GP_OPT_TILE_PX override (0 = library default)")
+    ap.add_argument("--pipeline", type=int, default=0, help="GP_OPT_PIPELINE override (0 = library default = 1 = serial)")
     ap.add_argument("--chunk-worlds", type=int, default=0,
                     help="worlds per gp_render_batch call (0 = as many as keep the planes under 40 GB)")
     ap.add_argument("--graph", action="store_true",
@@ -213,6 +216,12 @@ def run_b200(args):
         r.set_option(gp.GP_OPT_STAGE_CAP, args.stage_cap)
     if args.gather >= 0:
         r.set_option(gp.GP_OPT_GATHER, args.gather)
+    if args.variant >= 0:
+        r.set_option(gp.GP_OPT_VARIANT, args.variant)
+    if args.tile_px:
+        r.set_option(gp.GP_OPT_TILE_PX, args.tile_px)
+    if args.pipeline:
+        r.set_option(gp.GP_OPT_PIPELINE, args.pipeline)
     r.scene_upload(agents, quads, cam_height=cfg.cam_height, t_max=cfg.t_max)
     if cfg.pitch_deg_max > 0:
         r.cameras_set(torch.from_numpy(gs.gen_pitch(big, w0, cfg.n_worlds)).to(dev))
@@ -240,8 +249,11 @@ def run_b200(args):
             dist.barrier()
         torch.cuda.synchronize()
 
+    launches_per_step = 0
     for f in range(args.warmup):
+        l0 = r.launch_count()
         step(f)
+        launches_per_step = r.launch_count() - l0
     barrier()
     graphs = None
     if args.graph:                      # one graph per frame (each reads its own resident pose slice)
@@ -281,7 +293,7 @@ def run_b200(args):
     if graphs:
         # replays launch the captured kernels (1 update + cull + render per world chunk and step); per-kernel times
         # come from a short un-graphed pass after the timed region
-        launches = args.steps * (1 + 2 * len(chunks))
+        launches = args.steps * launches_per_step
         r.set_option(gp.GP_OPT_TIMING, 1)
         for k in (gp.GP_KERNEL_UPDATE, gp.GP_KERNEL_CULL, gp.GP_KERNEL_RENDER):
             r.kernel_time(k)
@@ -342,7 +354,9 @@ def run_b200(args):
     alg_bytes = npx * 12 + cfg.n_worlds * cfg.prims * 48 + cfg.views * 64
     r_ms, r_n = ktimes["render"]
     r_avg_ms = r_ms / max(1, r_n)
-    alg_bytes_launch = alg_bytes / len(chunks)                 # one k_render launch = one world chunk
+    steps_sampled = max(1, ktimes["update"][1])                # one pose update per step
+    render_launches_per_step = max(1.0, r_n / steps_sampled)   # render calls x pipeline chunks per call (GP_OPT_PIPELINE)
+    alg_bytes_launch = alg_bytes / render_launches_per_step    # one render launch = one world chunk of the pipeline
     achieved = alg_bytes_launch / (r_avg_ms * 1e-3) / 1e9
     traffic = None
     tpath = os.path.join(ROOT, "profiles", "r01_traffic.txt")      # from the committed ncu --set full capture
@@ -364,13 +378,14 @@ def run_b200(args):
         "mpixels_per_s": value * cfg.H * cfg.W / 1e6,
         "clocks": clocks,
         "gpu_launches": int(launches),
-        "kernels_ms_per_step": {k: v[0] / max(1, v[1]) * (len(chunks) if k != "update" else 1) for k, v in ktimes.items()},
+        "kernels_ms_per_step": {k: v[0] / steps_sampled for k, v in ktimes.items()},
         "kernel_samples": {k: int(v[1]) for k, v in ktimes.items()},
         "cuda_graph": bool(graphs),
         "roofline": {"bound": "hbm", "kernel": "k_render", "achieved": achieved, "peak": peak, "unit": "GB/s",
                      "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
                      "algorithmic_bytes_per_launch": alg_bytes_launch, "avg_launch_ms": r_avg_ms,
-                     "launches_per_step": len(chunks), "share_of_step": r_avg_ms * len(chunks) / step_ms},
+                     "launches_per_step": render_launches_per_step, "share_of_step": r_ms / steps_sampled / step_ms,
+                     "note": "the culls of later world chunks run concurrently with these launches on a second stream"},
         "roofline_step": {"t_hbm_ms": t_hbm_ms, "t_fp32_ms": t_fp32_ms, "frac_of_slower_roof": max(t_hbm_ms, t_fp32_ms) / step_ms,
                           "executed_tests": stats["executed_tests"], "listed_pairs": stats["listed_pairs"],
                           "tests_per_pixel": stats["executed_tests"] / npx, "fp32_peak_tflops": fp32_peak / 1e12,

@@ -52,6 +52,13 @@ enum {
     GP_OPT_GATHER = 6,      /* how a strip works off its list: 1 gather the overlapping entries first, one lane
                                per (flat quad, row); 0 entry by entry; -1 (default) chosen from the image size
                                and the primitives per world                                        */
+    GP_OPT_VARIANT = 8,     /* render pass: GP_VARIANT_RAY (pixel-major strips), GP_VARIANT_RASTER (primitive-major
+                               tiles with a depth buffer, PAPER.md:62 / :319) or -1 (default): chosen per launch
+                               shape from measurements.  Results are bit-identical.   */
+    GP_OPT_TILE_PX = 9,     /* raster variant: target pixels per tile; 0 = automatic                   */
+    GP_OPT_PIPELINE = 10,   /* n >= 1 world chunks per gp_render_batch; with n > 1 the culls of chunks 1.. run on a
+                               library-owned high-priority stream concurrently with the renders of earlier chunks.
+                               Default 1 (serial): the overlap measured slower on every workload */
     GP_OPT_SPHERES = 7      /* are records with shape == GP_SHAPE_SPHERE drawn?  -1 (default) automatic: yes iff the
                                uploaded scene held a sphere or gp_statics_update has run since the upload (its
                                records are device memory the host never inspects); 1 yes; 0 no: sphere records
@@ -64,6 +71,7 @@ enum {                      /* kernel ids of gp_kernel_time                     
     GP_KERNEL_RENDER = 2,   /* a3-a9 render pass (fast path)                                  */
     GP_KERNEL_BRUTE = 3     /* brute-force kernel                                             */
 };
+enum { GP_VARIANT_RAY = 0, GP_VARIANT_RASTER = 1 };
 enum {
     GP_PATH_FAST = 0,       /* cull + compaction, list staged in shared memory, strip render  */
     GP_PATH_BRUTE = 1       /* one thread per pixel, every primitive of the world, no culling */

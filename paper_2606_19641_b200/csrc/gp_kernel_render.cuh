@@ -25,6 +25,9 @@ struct RenderArgs {
     int ngr; uint32_t magicW;       // NG == 0: groups per whole strip when SR*W % 128 == 0 and W % 4 == 0 (else 0); ceil(2^32 / W)
     uint8_t *o_cls; int32_t *o_inst; float *o_depth; uint8_t *o_rgb;
     unsigned long long *stats;
+    // raster variant (gp_kernel_raster.cuh): SR = rows per tile, log2W = -1 unless W is a power of two
+    int ntiles;                     // tiles per view
+    float two_over_H, two_over_W;   // 2.0f / (float)H, 2.0f / (float)W: IEEE divisions done on the host (C2)
 };
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -177,8 +180,10 @@ __device__ __forceinline__ void slab_select(const float4 &g0, float dlx, float d
         else if (loy == tn) face = 2 + (dly > 0.0f ? 0 : 1);
         else face = 4 + (dz > 0.0f ? 0 : 1);
         const unsigned long long key = ((unsigned long long)__float_as_uint(tn) << 32) | klow | face;   // C6
-        if (ATOMIC) atomicMin(kp, key);
-        else if (key < *kp) *kp = key;
+        if (key < *kp) {                                // (racy pre-read under ATOMIC: keys only ever decrease)
+            if (ATOMIC) atomicMin(kp, key);
+            else *kp = key;
+        }
     }
 }
 
@@ -386,9 +391,13 @@ __device__ __forceinline__ unsigned strip_batch(const StripBatchCtx &c, const ui
 // flat quads get one lane per (entry, row) (fewer instructions when many entries meet a strip: small images, dense
 // scenes); false: entry by entry as the ballot finds them, the warp spread over each entry's rectangle (1 % faster
 // when lists are short and the kernel is store-bound).  The host picks (gp_lib.cu).
+#ifndef GP_RENDER_DYNAMIC
+#define GP_RENDER_DYNAMIC 1
+#endif
 template <bool STATS, int NG, bool SPH, bool GATHER>
 __global__ void __launch_bounds__(GP_RENDER_WARPS * 32, GP_RENDER_MIN_CTAS)
 k_render(SceneConst sc, RenderArgs ra) {
+    constexpr bool DYN = GP_RENDER_DYNAMIC != 0;
     extern __shared__ __align__(16) unsigned char smem[];
     const int view = blockIdx.x;
     const int H = ra.H, W = ra.W, SR = ra.SR;
@@ -427,9 +436,11 @@ k_render(SceneConst sc, RenderArgs ra) {
         }
     }
     // tables (contract C2-C4), overlapped with the bulk copies
-    for (int j = threadIdx.x; j < W; j += blockDim.x) s_col[j] = pix_s(j, W, ra.th);
+    // (2 / W and 2 / H are IEEE divisions done once on the host: the same fp32 numbers pix_s / pix_v form)
+    for (int j = threadIdx.x; j < W; j += blockDim.x)
+        s_col[j] = c_mul(c_sub(c_mul(c_add((float)j, 0.5f), ra.two_over_W), 1.0f), ra.th);
     for (int i = threadIdx.x; i < H; i += blockDim.x) {
-        const float v = pix_v(i, H, ra.tv);
+        const float v = c_mul(c_sub(1.0f, c_mul(c_add((float)i, 0.5f), ra.two_over_H)), ra.tv);
         const float dz = c_fma(v, vh.cp, vh.sp);
         const float inv_z = c_rcp(dz);
         float tg = -1.0f;
@@ -457,10 +468,13 @@ k_render(SceneConst sc, RenderArgs ra) {
     const EntryGeo *g_geo = ra.geo + (size_t)view * ra.cap;
     const EntryAux *g_aux = ra.aux + (size_t)view * ra.cap;
     bool list_ready = false;
-    for (;;) {
-        int strip = 0;
-        if (lane == 0) strip = atomicAdd(s_next, 1);
-        strip = __shfl_sync(0xffffffffu, strip, 0);
+    const int n_warps = blockDim.x >> 5;
+    for (int strip_it = warp;; strip_it += n_warps) {
+        int strip = strip_it;
+        if (DYN) {                                                      // dynamic hand-out (balances long lists)
+            if (lane == 0) strip = atomicAdd(s_next, 1);
+            strip = __shfl_sync(0xffffffffu, strip, 0);
+        }
         if (strip >= n_strips) break;
         if (strip >= n_free && !list_ready) { mbar_wait(bar, 0); list_ready = true; }
         const int nn = strip < n_free ? 0 : n;                      // entries to scan for this strip

@@ -10,6 +10,7 @@
 #include "gp_kernels_basic.cuh"
 #include "gp_kernel_cull.cuh"
 #include "gp_kernel_render.cuh"
+#include "gp_kernel_raster.cuh"
 
 using namespace gp;
 
@@ -31,12 +32,15 @@ struct gp_ctx {
     size_t scratch_views = 0; int scratch_cap = 0;
     unsigned long long *d_stats = nullptr;
     int opt_path = GP_PATH_FAST, opt_stats = 0, opt_timing = 0, opt_stage_cap = GP_STAGE_CAP, opt_strip_px = 0, opt_gather = -1, opt_spheres = -1;
+    int opt_variant = -1, opt_tile_px = 0, opt_pipeline = 1;
+    cudaStream_t aux_stream = nullptr;                           // culls of later chunks run here (render_device)
+    std::vector<cudaEvent_t> pipe_ev;
     struct Timed { int kernel; cudaEvent_t a, b; };
     std::vector<Timed> timed;                                    // GP_OPT_TIMING records
     std::vector<cudaEvent_t> ev_pool;
     uint64_t launches = 0;
     unsigned timing_seq[4] = {0, 0, 0, 0};
-    size_t render_smem_set = 0;
+    size_t render_smem_set = 0, raster_smem_set = 0;
     // gp_render_batch_host staging
     float *d_pose = nullptr;
     unsigned char *d_out[2] = {nullptr, nullptr}; size_t d_out_bytes = 0;
@@ -150,6 +154,8 @@ extern "C" int gp_destroy(gp_ctx *c) {
     for (auto &t : c->timed) { cudaEventDestroy(t.a); cudaEventDestroy(t.b); }
     for (auto e : c->ev_pool) cudaEventDestroy(e);
     if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
+    if (c->aux_stream) cudaStreamDestroy(c->aux_stream);
+    for (auto e : c->pipe_ev) cudaEventDestroy(e);
     if (c->h_stage) cudaFreeHost(c->h_stage);
     cudaFree(c->d_stats);
     }
@@ -176,6 +182,15 @@ extern "C" int gp_set_option(gp_ctx *c, int key, int value) {
         case GP_OPT_GATHER:
             if (value < -1 || value > 1) return GP_ERR_ARG;
             c->opt_gather = value; return GP_OK;
+        case GP_OPT_VARIANT:
+            if (value < -1 || value > GP_VARIANT_RASTER) return GP_ERR_ARG;
+            c->opt_variant = value; return GP_OK;
+        case GP_OPT_PIPELINE:
+            if (value < 1 || value > 64) return GP_ERR_ARG;
+            c->opt_pipeline = value; return GP_OK;
+        case GP_OPT_TILE_PX:
+            if (value < 0 || value > 16384) return GP_ERR_ARG;
+            c->opt_tile_px = value; return GP_OK;
         case GP_OPT_SPHERES:
             if (value < -1 || value > 1) return GP_ERR_ARG;
             c->opt_spheres = value; return GP_OK;
@@ -421,6 +436,32 @@ static bool plan_render(const gp_ctx *c, const SceneConst &sc, int H, int W, Ren
     return smem <= 227 * 1024;
 }
 
+// Launch shape of the raster variant: rows per tile TR (a multiple of the strip alignment, of 4 when > 4 so that the
+// 4 x 8 walk of a box stays inside whole row blocks), tiles per view, warps per CTA, shared memory.
+struct RasterPlan { int TR, ntiles, nwarps, log2LC, wshift, scap; uint32_t magicW; size_t smem; };
+static bool plan_raster(const gp_ctx *c, const SceneConst &sc, int H, int W, RasterPlan &pl) {
+    const int align = (W & 1) ? 4 : (W & 2) ? 2 : 1;           // tiles start on a multiple of 4 pixels
+    const int tile_px = c->opt_tile_px > 0 ? c->opt_tile_px : 2048;
+    int TR = tile_px / W;
+    if (TR >= 4) TR &= ~3;
+    TR -= TR % align;
+    if (TR < align) TR = align;
+    if (TR > H) TR = ((H + align - 1) / align) * align;        // one (ragged) tile
+    pl.TR = TR;
+    pl.ntiles = (H + TR - 1) / TR;
+    const int LR = TR >= 4 ? 4 : TR >= 2 ? 2 : 1;
+    pl.log2LC = LR == 4 ? 3 : LR == 2 ? 4 : 5;
+    int log2W = 0;
+    while ((1 << log2W) < W) ++log2W;
+    pl.wshift = (1 << log2W) == W ? log2W : -1;
+    pl.magicW = (uint32_t)((0x100000000ull + (unsigned)W - 1) / (unsigned)W);
+    pl.scap = std::min(sc.P, c->opt_stage_cap);
+    const int groups = (TR * W + 127) / 128;
+    pl.nwarps = groups >= 8 ? GP_RASTER_WARPS : groups >= 2 ? 2 : 1;
+    pl.smem = 48 + (size_t)pl.scap * 64 + (size_t)TR * 16 + (size_t)((W + 3) & ~3) * 4 + (size_t)TR * W * 8;
+    return pl.smem <= 227 * 1024;
+}
+
 // Enqueue cull + render (or the brute-force kernel) for a world range into DEVICE planes.
 static int render_device(gp_ctx *c, int world_begin, int n_worlds, int H, int W, float fov_rad,
                          uint8_t *d_class, int32_t *d_instance, float *d_depth, uint8_t *d_rgb,
@@ -441,7 +482,12 @@ static int render_device(gp_ctx *c, int world_begin, int n_worlds, int H, int W,
     // fast path: every view (H*W pixels) must start 16-byte aligned in the 32-bit planes, and one warp's strip
     // must fit shared memory (it does not for e.g. 4096 x 4094: odd widths force 2- or 4-row strips)
     RenderPlan pl{};
-    const bool fast_ok = W >= 4 && !(((long long)H * W) & 3) && plan_render(c, sc, H, W, pl);
+    RasterPlan rp{};
+    int variant = c->opt_variant;
+    if (variant < 0) variant = GP_VARIANT_RAY;
+    const bool size_ok = W >= 4 && !(((long long)H * W) & 3);
+    if (variant == GP_VARIANT_RASTER && !(size_ok && plan_raster(c, sc, H, W, rp))) variant = GP_VARIANT_RAY;
+    const bool fast_ok = size_ok && (variant == GP_VARIANT_RASTER || plan_render(c, sc, H, W, pl));
     if (c->opt_path == GP_PATH_BRUTE || !fast_ok) {
         const int HW = H * W;
         dim3 grid((unsigned)views, (unsigned)std::min((HW + 255) / 256, 65535));
@@ -456,44 +502,110 @@ static int render_device(gp_ctx *c, int world_begin, int n_worlds, int H, int W,
     }
     int rc = ensure_scratch(c, views);
     if (rc != GP_OK) return rc;
-    {
-        LaunchTimer lt(c, GP_KERNEL_CULL, stream);
-        const int gpw = (sc.A * sc.C + kCullWarps - 1) / kCullWarps;   // CTAs per world
-        k_cull<<<(unsigned)((size_t)n_worlds * gpw), kCullWarps * 32, 0, stream>>>(
-            sc, c->d_prims, c->d_pitch, world_begin, gpw, H, W, th, tv,
-                                                    c->d_hdr, c->d_geo, c->d_aux, c->scratch_cap, stats);
-    }
-    c->launches += 1;
-    CK(cudaGetLastError());
 
-    RenderArgs ra;
-    ra.hdr = c->d_hdr; ra.geo = c->d_geo; ra.aux = c->d_aux; ra.meta = c->d_meta;
-    ra.cap = c->scratch_cap; ra.scap = pl.scap; ra.world_begin = world_begin; ra.H = H; ra.W = W; ra.th = th; ra.tv = tv;
-    ra.SR = pl.SR; ra.log2LC = pl.log2LC; ra.log2W = pl.log2W; ra.ngr = pl.ngr; ra.magicW = pl.magicW;
-    ra.o_cls = d_class; ra.o_inst = d_instance; ra.o_depth = d_depth; ra.o_rgb = d_rgb; ra.stats = stats;
-    const int ng = pl.ng, nwarps = pl.nwarps, gather = pl.gather;
-    const size_t smem = pl.smem;
+    // ---- pipeline over world chunks: the cull of chunk i + 1 runs on a library-owned high-priority stream while chunk i
+    // renders on the caller's stream (the cull is bound by instruction issue and latency, the render by HBM stores,
+    // so they overlap well; serially the cull costs 8 % of the paper-scale step).  Fork / join by events, capturable in
+    // a CUDA graph.  Every chunk has its own slice of the per-view scratch, so culls may run arbitrarily far ahead.
+    const int vpw = sc.A * sc.C;                                       // views per world
+    int n_chunks = c->opt_pipeline;                                    // default 1: measured slower than serial
+    n_chunks = std::min(n_chunks, n_worlds);
+    if (stats || n_chunks < 1) n_chunks = 1;
+    const int wpc = (n_worlds + n_chunks - 1) / n_chunks;              // worlds per chunk
+    n_chunks = (n_worlds + wpc - 1) / wpc;
+    cudaStream_t cull_stream = stream;
+    if (n_chunks > 1) {
+        if (!c->aux_stream) {
+            int lo = 0, hi = 0;
+            CK(cudaDeviceGetStreamPriorityRange(&lo, &hi));
+            CK(cudaStreamCreateWithPriority(&c->aux_stream, cudaStreamNonBlocking, hi));
+        }
+        while ((int)c->pipe_ev.size() < n_chunks + 1) {
+            cudaEvent_t e;
+            CK(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+            c->pipe_ev.push_back(e);
+        }
+        cull_stream = c->aux_stream;
+        CK(cudaEventRecord(c->pipe_ev[n_chunks], stream));             // fork: the culls see everything enqueued so far
+        CK(cudaStreamWaitEvent(cull_stream, c->pipe_ev[n_chunks], 0));
+    }
+    const int gpw = (vpw + kCullWarps - 1) / kCullWarps;               // cull CTAs per world
+    auto launch_cull = [&](int ci, cudaStream_t st) -> int {
+        const int w0 = ci * wpc, nw = std::min(wpc, n_worlds - w0);
+        const size_t v0 = (size_t)w0 * vpw;
+        {
+            LaunchTimer lt(c, GP_KERNEL_CULL, st);
+            k_cull<<<(unsigned)((size_t)nw * gpw), kCullWarps * 32, 0, st>>>(
+                sc, c->d_prims, c->d_pitch, world_begin + w0, gpw, H, W, th, tv, c->d_hdr + v0,
+                c->d_geo + v0 * c->scratch_cap, c->d_aux + v0 * c->scratch_cap, c->scratch_cap, stats);
+        }
+        c->launches += 1;
+        CK(cudaGetLastError());
+        return GP_OK;
+    };
+
+    RenderArgs ra{};
+    ra.meta = c->d_meta;
+    ra.two_over_H = 2.0f / (float)H; ra.two_over_W = 2.0f / (float)W;
+    ra.cap = c->scratch_cap; ra.H = H; ra.W = W; ra.th = th; ra.tv = tv; ra.stats = stats;
     typedef void (*RenderFn)(SceneConst, RenderArgs);
-#define GP_FNS(ST, SP, GA) {k_render<ST, 0, SP, GA>, k_render<ST, 1, SP, GA>, k_render<ST, 2, SP, GA>, k_render<ST, 4, SP, GA>}
-    static const RenderFn fns[2][2][2][4] = {      // [gather][spheres][stats][ng index]
-        {{GP_FNS(false, false, false), GP_FNS(true, false, false)}, {GP_FNS(false, true, false), GP_FNS(true, true, false)}},
-        {{GP_FNS(false, false, true), GP_FNS(true, false, true)}, {GP_FNS(false, true, true), GP_FNS(true, true, true)}}};
-#undef GP_FNS
-    if (smem > c->render_smem_set) {
-        for (int ga = 0; ga < 2; ++ga)
+    RenderFn fn = nullptr;
+    unsigned ctas_per_view = 1, block = 0;
+    size_t smem = 0;
+    if (variant == GP_VARIANT_RASTER) {
+        ra.scap = rp.scap; ra.SR = rp.TR; ra.log2LC = rp.log2LC; ra.log2W = rp.wshift; ra.magicW = rp.magicW; ra.ntiles = rp.ntiles;
+        static const RenderFn rfns[2][2] = {{k_raster<false, false>, k_raster<true, false>},
+                                            {k_raster<false, true>, k_raster<true, true>}};     // [spheres][stats]
+        if (rp.smem > c->raster_smem_set) {
             for (int f = 0; f < 2; ++f)
                 for (int st = 0; st < 2; ++st)
-                    for (int g = 0; g < 4; ++g)
-                        CK(cudaFuncSetAttribute(fns[ga][f][st][g], cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        c->render_smem_set = smem;
+                    CK(cudaFuncSetAttribute(rfns[f][st], cudaFuncAttributeMaxDynamicSharedMemorySize, (int)rp.smem));
+            c->raster_smem_set = rp.smem;
+        }
+        if (views * (size_t)rp.ntiles > 0x7fffffffull) return GP_ERR_ARG;
+        fn = rfns[spheres ? 1 : 0][stats ? 1 : 0];
+        ctas_per_view = (unsigned)rp.ntiles; block = (unsigned)rp.nwarps * 32; smem = rp.smem;
+    } else {
+        ra.scap = pl.scap; ra.SR = pl.SR; ra.log2LC = pl.log2LC; ra.log2W = pl.log2W; ra.ngr = pl.ngr; ra.magicW = pl.magicW;
+#define GP_FNS(ST, SP, GA) {k_render<ST, 0, SP, GA>, k_render<ST, 1, SP, GA>, k_render<ST, 2, SP, GA>, k_render<ST, 4, SP, GA>}
+        static const RenderFn fns[2][2][2][4] = {      // [gather][spheres][stats][ng index]
+            {{GP_FNS(false, false, false), GP_FNS(true, false, false)}, {GP_FNS(false, true, false), GP_FNS(true, true, false)}},
+            {{GP_FNS(false, false, true), GP_FNS(true, false, true)}, {GP_FNS(false, true, true), GP_FNS(true, true, true)}}};
+#undef GP_FNS
+        if (pl.smem > c->render_smem_set) {
+            for (int ga = 0; ga < 2; ++ga)
+                for (int f = 0; f < 2; ++f)
+                    for (int st = 0; st < 2; ++st)
+                        for (int g = 0; g < 4; ++g)
+                            CK(cudaFuncSetAttribute(fns[ga][f][st][g], cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem));
+            c->render_smem_set = pl.smem;
+        }
+        fn = fns[pl.gather][spheres ? 1 : 0][stats ? 1 : 0][pl.ng == 4 ? 3 : pl.ng];
+        block = (unsigned)pl.nwarps * 32; smem = pl.smem;
     }
-    {
-        LaunchTimer lt(c, GP_KERNEL_RENDER, stream);
-        const RenderFn fn = fns[gather][spheres ? 1 : 0][stats ? 1 : 0][ng == 4 ? 3 : ng];
-        fn<<<dim3((unsigned)views), dim3(nwarps * 32), smem, stream>>>(sc, ra);
+    const size_t HW = (size_t)H * W;
+    rc = launch_cull(0, stream);                                       // chunk 0: nothing to overlap with yet
+    if (rc != GP_OK) return rc;
+    for (int ci = 1; ci < n_chunks; ++ci) {                            // the other culls run ahead on the side stream
+        rc = launch_cull(ci, cull_stream);
+        if (rc != GP_OK) return rc;
+        CK(cudaEventRecord(c->pipe_ev[ci], cull_stream));
     }
-    c->launches += 1;
-    CK(cudaGetLastError());
+    for (int ci = 0; ci < n_chunks; ++ci) {
+        const int w0 = ci * wpc, nw = std::min(wpc, n_worlds - w0);
+        const size_t v0 = (size_t)w0 * vpw, nv = (size_t)nw * vpw;
+        if (ci > 0) CK(cudaStreamWaitEvent(stream, c->pipe_ev[ci], 0));  // join (the last one joins the side stream for good)
+        ra.hdr = c->d_hdr + v0; ra.geo = c->d_geo + v0 * c->scratch_cap; ra.aux = c->d_aux + v0 * c->scratch_cap;
+        ra.world_begin = world_begin + w0;
+        ra.o_cls = d_class + v0 * HW; ra.o_inst = d_instance + v0 * HW; ra.o_depth = d_depth + v0 * HW;
+        ra.o_rgb = d_rgb ? d_rgb + v0 * 3 * HW : nullptr;
+        {
+            LaunchTimer lt(c, GP_KERNEL_RENDER, stream);
+            fn<<<dim3((unsigned)(nv * ctas_per_view)), dim3(block), smem, stream>>>(sc, ra);
+        }
+        c->launches += 1;
+        CK(cudaGetLastError());
+    }
     return GP_OK;
 }
 

@@ -21,13 +21,14 @@ def world_prims(agents, quads):
     return np.concatenate([agents, quads], axis=1) if quads is not None and quads.size else agents
 
 
-def gpu_render(renderer, cfg, world_begin, n_worlds, path=0, rgb=True, H=None, W=None, fov=None, gather=None):
+def gpu_render(renderer, cfg, world_begin, n_worlds, path=0, rgb=True, H=None, W=None, fov=None, gather=None, variant=None):
     """Render a world range through the C ABI; returns numpy planes."""
     import torch
     from paper_2606_19641_b200 import gp
     H = H or cfg.H; W = W or cfg.W
     renderer.set_option(gp.GP_OPT_PATH, path)
     renderer.set_option(gp.GP_OPT_GATHER, -1 if gather is None else gather)
+    renderer.set_option(gp.GP_OPT_VARIANT, -1 if variant is None else variant)
     outs = renderer.alloc_outputs(n_worlds * cfg.agents * renderer.n_cams, H, W, rgb=rgb)
     for t in outs:
         if t is not None:
