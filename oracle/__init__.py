@@ -28,6 +28,21 @@ class Cam(ctypes.Structure):
     _fields_ = [("cd", ctypes.c_float), ("sd", ctypes.c_float), ("mount", ctypes.c_float)]
 
 
+class DynParams(ctypes.Structure):
+    """Limits of the jerk-actuated kinematic bicycle (gp_sim_oracle.c)."""
+    _fields_ = [("dt", ctypes.c_float), ("a_lon_max", ctypes.c_float), ("a_lat_max", ctypes.c_float),
+                ("v_max", ctypes.c_float), ("steer_max", ctypes.c_float), ("steer_rate_max", ctypes.c_float),
+                ("v_eps", ctypes.c_float), ("extent", ctypes.c_float)]
+
+
+def make_dyn_params(dt=0.1, a_lon_max=6.0, a_lat_max=4.0, v_max=20.0, steer_max=0.6, steer_rate_max=0.8, v_eps=0.5,
+                    extent=0.0) -> DynParams:
+    p = DynParams()
+    p.dt, p.a_lon_max, p.a_lat_max, p.v_max = dt, a_lon_max, a_lat_max, v_max
+    p.steer_max, p.steer_rate_max, p.v_eps, p.extent = steer_max, steer_rate_max, v_eps, extent
+    return p
+
+
 PALETTE = ((135, 206, 235), (90, 90, 90), (240, 240, 240), (40, 80, 220),
            (220, 60, 60), (240, 160, 40), (150, 110, 70), (250, 240, 80))
 
@@ -68,6 +83,10 @@ def lib():
         L.orc_shadow_view.restype = ci
         L.orc_polyline_quads.argtypes = [vp, ci, ci, cf, cf, ci, ci, vp]
         L.orc_polyline_quads.restype = ci
+        L.orc_dynamics_step.argtypes = [ctypes.POINTER(DynParams), ci, vp, vp, vp, vp]
+        L.orc_dynamics_step.restype = ci
+        L.orc_observe_vec.argtypes = [vp, ci, ci, vp, ci, ci, cf, vp, vp, vp, vp]
+        L.orc_observe_vec.restype = ci
         _lib = L
     return _lib
 
@@ -148,3 +167,39 @@ def render_views(world_prims, views, H, W, params=None, pitch_cs=None, rgb=True,
         return [one(v) for v in views]
     with ThreadPoolExecutor(max_workers=threads) as ex:
         return list(ex.map(one, views))
+
+
+def dynamics_step(params, action, half_len, state, pose):
+    """One step of the jerk bicycle for n agents (fp64 inside, fp32 in / out).  action int32 [n], half_len fp32 [n],
+    state fp32 [n][8] = (v, a_lon, a_lat, steer, psi, -, -, -), pose fp32 [n][4] = (x, y, cos psi, sin psi).
+    Returns (new_state, new_pose); the inputs are not modified."""
+    action = np.ascontiguousarray(action, dtype=np.int32).reshape(-1)
+    n = action.size
+    half_len = np.ascontiguousarray(half_len, dtype=np.float32).reshape(n)
+    st = np.array(state, dtype=np.float32, copy=True).reshape(n, 8)
+    ps = np.array(pose, dtype=np.float32, copy=True).reshape(n, 4)
+    rc = lib().orc_dynamics_step(ctypes.byref(params), n, action.ctypes.data, half_len.ctypes.data,
+                                 st.ctypes.data, ps.ctypes.data)
+    if rc != 0:
+        raise ValueError("orc_dynamics_step: bad arguments (%d)" % rc)
+    return st.reshape(np.shape(state)), ps.reshape(np.shape(pose))
+
+
+def observe_vec(world_prims, n_agents, speed, K, M, radius=100.0):
+    """O_vec of every agent of every world.  world_prims [Wn][P] 48-byte records (agents first), speed fp32 [Wn][A].
+    Returns dict(agent_idx i32 [Wn][A][K], agent_feat f32 [Wn][A][K][8], road_idx i32 [Wn][A][M], road_feat f32
+    [Wn][A][M][8])."""
+    prims = np.ascontiguousarray(world_prims)
+    assert prims.ndim == 2 and prims.dtype.itemsize == _PRIM_BYTES
+    Wn, P = prims.shape
+    A = int(n_agents)
+    speed = np.ascontiguousarray(speed, dtype=np.float32).reshape(Wn, A)
+    out = {"agent_idx": np.empty((Wn, A, K), np.int32), "agent_feat": np.empty((Wn, A, K, 8), np.float32),
+           "road_idx": np.empty((Wn, A, M), np.int32), "road_feat": np.empty((Wn, A, M, 8), np.float32)}
+    for w in range(Wn):
+        rc = lib().orc_observe_vec(prims[w].ctypes.data, P, A, speed[w].ctypes.data, int(K), int(M), float(radius),
+                                   out["agent_idx"][w].ctypes.data, out["agent_feat"][w].ctypes.data,
+                                   out["road_idx"][w].ctypes.data, out["road_feat"][w].ctypes.data)
+        if rc != 0:
+            raise ValueError("orc_observe_vec: bad arguments")
+    return out

@@ -11,6 +11,7 @@ import subprocess
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 SRC = os.path.join(HERE, "gp_oracle.c")
+SRCS = [SRC, os.path.join(HERE, "gp_sim_oracle.c")]      # renderer; dynamics + vectorised observation (NEXT-4)
 LIB = os.path.join(HERE, "libgp_oracle.so")
 CFLAGS = ["-O2", "-ffp-contract=off", "-fno-fast-math", "-mfma", "-std=c99",
           "-Wall", "-Wextra", "-shared", "-fPIC"]
@@ -18,10 +19,10 @@ CFLAGS = ["-O2", "-ffp-contract=off", "-fno-fast-math", "-mfma", "-std=c99",
 
 def build(force: bool = False) -> str:
     if (not force and os.path.exists(LIB)
-            and os.path.getmtime(LIB) >= os.path.getmtime(SRC)):
+            and all(os.path.getmtime(LIB) >= os.path.getmtime(x) for x in SRCS)):
         return LIB
     tmp = LIB + ".tmp.%d" % os.getpid()
-    subprocess.check_call(["gcc", *CFLAGS, SRC, "-o", tmp, "-lm"])
+    subprocess.check_call(["gcc", *CFLAGS, *SRCS, "-o", tmp, "-lm"])
     os.replace(tmp, LIB)
     return LIB
 
