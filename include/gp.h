@@ -69,7 +69,9 @@ enum {                      /* kernel ids of gp_kernel_time                     
     GP_KERNEL_UPDATE = 0,   /* a0 pose update + shading table                                 */
     GP_KERNEL_CULL = 1,     /* a1 camera setup + a2 frustum cull and compaction               */
     GP_KERNEL_RENDER = 2,   /* a3-a9 render pass (fast path)                                  */
-    GP_KERNEL_BRUTE = 3     /* brute-force kernel                                             */
+    GP_KERNEL_BRUTE = 3,    /* brute-force kernel                                             */
+    GP_KERNEL_DYNAMICS = 4, /* gp_dynamics_step                                               */
+    GP_KERNEL_OBSERVE = 5   /* gp_observe_vec                                                 */
 };
 enum { GP_VARIANT_RAY = 0, GP_VARIANT_RASTER = 1 };
 enum {
@@ -195,6 +197,55 @@ int gp_render_batch(gp_ctx *ctx, int world_begin, int n_worlds, int agents, int 
 int gp_render_batch_host(gp_ctx *ctx, const float *h_pose, int world_begin, int n_worlds, int agents,
                          int H, int W, float fov_rad, uint8_t *h_class, int32_t *h_instance,
                          float *h_depth, uint8_t *h_rgb, void *stream);
+
+/* ---- the step either side of the render --------------------------------------------------- */
+
+/* Limits of the jerk-actuated kinematic bicycle ("accelerations clipped to g-force limits, speed clipped
+ * to the speed limit, and the steering angle and its rate bounded"; the paper gives no numbers: caller's choice). */
+typedef struct {
+    float dt;               /* step, s (the paper simulates at 0.1 s)                                  */
+    float a_lon_max;        /* |longitudinal acceleration| limit, m/s^2                                */
+    float a_lat_max;        /* |lateral acceleration| limit, m/s^2                                     */
+    float v_max;            /* speed limit, m/s: speed is clipped to [0, v_max] (no reversing)         */
+    float steer_max;        /* |steering angle| limit, rad                                             */
+    float steer_rate_max;   /* |steering rate| limit, rad/s                                            */
+    float v_eps;            /* the curvature demand a_lat / v^2 uses max(v, v_eps), m/s (> 0)          */
+    float extent;           /* > 0: positions wrap onto the torus [-extent/2, extent/2); 0: no wrap    */
+} gp_dyn_params;
+
+/* One simulation step of every agent, on the device (DESIGN.md "Dynamics contract" D1-D6), fused with
+ * the pose update a0 of gp_agents_update:
+ *   d_action DEVICE int32 [Wn][A]: one of the twelve actions, = 3 * i_lon + i_lat with longitudinal jerk
+ *            {-15, -4, 0, 4}[i_lon] and lateral jerk {-4, 0, 4}[i_lat] m/s^3; other values leave the agent untouched
+ *   d_state  DEVICE fp32 [Wn][A][8], in / out: speed v, a_lon, a_lat, steering angle, heading psi in [-pi, pi), 3 unused
+ *   d_pose   DEVICE fp32 [Wn][A][4], in / out: (cx, cy, cos psi, sin psi) — the layout gp_agents_update takes
+ * Jerks -> accelerations (clipped) -> speed (clipped to [0, v_max]) -> steering angle demanded by a_lat = v^2 kappa with
+ * kappa = tan(steer) / L, wheelbase L = 0.6 * vehicle length (2 hx of the agent's record), bounded in rate and
+ * magnitude -> heading -> position (new speed and heading; optional torus wrap).  The new poses are also written into
+ * the scene (agent records + shading table), so gp_render_batch can follow with no host transfer.
+ * fp32 arithmetic with atanf / tanf / sincosf.  Both pointers 16-byte aligned. */
+int gp_dynamics_step(gp_ctx *ctx, const gp_dyn_params *params, const int32_t *d_action, float *d_state,
+                     float *d_pose, void *stream);
+
+/* The vectorised observation O_vec of every agent (DESIGN.md "Observation contract" O1-O3), from the
+ * scene as it stands (agent records as last written by gp_agents_update / gp_dynamics_step; statics).  Ego frame of
+ * agent i: origin at its box centre, x along its heading, y to its left.
+ *   d_state      DEVICE fp32 [Wn][A][8]: only element 0 (signed speed) of each agent is read
+ *   d_agent_idx  DEVICE int32 [Wn][A][K]: the K nearest other agents with squared centre distance <= radius^2, ascending
+ *                (distance, index); -1 pads.  "the nearest K within 100 m"
+ *   d_agent_feat DEVICE fp32 [Wn][A][K][8]: rel x, rel y, length, width, cos and sin of the relative heading, relative
+ *                signed speed v_j - v_i, 1; zeros pad
+ *   d_road_idx   DEVICE int32 [Wn][A][M]: primitive indices (>= A) of the M nearest road segments — static box records
+ *                with hz == 0 — by their centre, within the radius; -1 pads
+ *   d_road_feat  DEVICE fp32 [Wn][A][M][8]: rel x, rel y of the centre, length, cos and sin of the segment's direction in
+ *                the ego frame, type (= cls), 1, 0; zeros pad
+ * K = 0 or M = 0 skips that part (its pointers may then be NULL).  The paper retrieves segments "from a spatial hash";
+ * here every segment of the agent's world is examined from shared memory (a few hundred per world), which returns the
+ * same set.  All arithmetic is fp32 add / mul / fma in a fixed order: results are bit-exact against the oracle.
+ * K, M <= 1024; GP_ERR_ARG if a world's records do not fit shared memory (more than ~6000 primitives per world).
+ * Feature pointers 16-byte aligned. */
+int gp_observe_vec(gp_ctx *ctx, const float *d_state, int K, int M, float radius, int32_t *d_agent_idx,
+                   float *d_agent_feat, int32_t *d_road_idx, float *d_road_feat, void *stream);
 
 /* Counters of the last gp_render_batch issued with GP_OPT_STATS = 1 (synchronises the device):
  * executed_tests = ray/primitive slab tests actually evaluated, listed_pairs = (view, primitive)

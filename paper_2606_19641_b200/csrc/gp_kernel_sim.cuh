@@ -1,0 +1,174 @@
+// gp_kernel_sim.cuh — the step either side of the render: the jerk-actuated kinematic
+// bicycle that advances the agents fused with the pose update a0, and the vectorised observation
+// O_vec.  Contracts: DESIGN.md "Dynamics contract" D1-D6 (fp32 with libm atanf / tanf / sincosf:
+// parity with the fp64 oracle by tolerance) and "Observation contract" O1-O3 (fp32 add / mul / fma only, explicit
+// round-to-nearest intrinsics: bit-exact).
+#pragma once
+#include "gp_device.cuh"
+#include "gp_kernels_basic.cuh"
+
+namespace gp {
+
+__device__ __forceinline__ float clipf(float x, float lo, float hi) { return fminf(fmaxf(x, lo), hi); }
+
+// D1-D6 + a0.  One thread per agent: reads its action, kinematic state and pose, writes the new state and pose, the
+// agent's primitive record (centre, heading) and its shading table, so the renderer can be called right after with
+// no host transfer and no separate pose-update launch.
+__global__ void k_dynamics_step(SceneConst sc, gp_dyn_params par, const int32_t *__restrict__ action,
+                                float4 *__restrict__ state /* [n][2]: (v a_lon a_lat steer) (psi - - -) */,
+                                float4 *__restrict__ pose, gp_prim *__restrict__ prims, PrimMeta *__restrict__ meta) {
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const size_t n = (size_t)sc.Wn * sc.A;
+    if (i >= n) return;
+    const int a = __ldg(&action[i]);
+    if (a < 0 || a >= 12) return;                                   // invalid action: the agent is left untouched
+    const size_t w = i / sc.A, ag = i % sc.A;
+    gp_prim *p = &prims[w * sc.P + ag];
+    const float4 s0 = state[2 * i], s1 = state[2 * i + 1], ps = pose[i];
+    const int il = a / 3, it = a - 3 * il;
+    const float jlon = il == 0 ? -15.0f : il == 1 ? -4.0f : il == 2 ? 0.0f : 4.0f;
+    const float jlat = it == 0 ? -4.0f : it == 1 ? 0.0f : 4.0f;
+    const float dt = par.dt;
+    float v = s0.x, a_lon = s0.y, a_lat = s0.z, steer = s0.w, psi = s1.x, x = ps.x, y = ps.y;
+    a_lon = clipf(fmaf(jlon, dt, a_lon), -par.a_lon_max, par.a_lon_max);                 // D1
+    a_lat = clipf(fmaf(jlat, dt, a_lat), -par.a_lat_max, par.a_lat_max);
+    v = clipf(fmaf(a_lon, dt, v), 0.0f, par.v_max);                                      // D2
+    const float L = 0.6f * (2.0f * p->hx);                                               // D3: wheelbase
+    const float vv = fmaxf(v, par.v_eps);
+    const float want = atanf(L * a_lat / (vv * vv));
+    const float dmax = par.steer_rate_max * dt;
+    steer = steer + clipf(want - steer, -dmax, dmax);
+    steer = clipf(steer, -par.steer_max, par.steer_max);
+    psi = fmaf(v * (tanf(steer) / L), dt, psi);                                          // D4
+    const float PI = 3.14159265358979323846f;
+    if (psi >= PI) psi -= 2.0f * PI;
+    if (psi < -PI) psi += 2.0f * PI;
+    float sn, c;
+    sincosf(psi, &sn, &c);
+    x = fmaf(v * c, dt, x);                                                              // D5
+    y = fmaf(v * sn, dt, y);
+    if (par.extent > 0.0f) {                                                             // D6
+        const float E = par.extent, h = 0.5f * E;
+        if (x >= h) x -= E;
+        if (x < -h) x += E;
+        if (y >= h) y -= E;
+        if (y < -h) y += E;
+    }
+    state[2 * i] = make_float4(v, a_lon, a_lat, steer);
+    state[2 * i + 1] = make_float4(psi, s1.y, s1.z, s1.w);
+    pose[i] = make_float4(x, y, c, sn);
+    p->cx = x; p->cy = y; p->cos_yaw = c; p->sin_yaw = sn;                               // a0
+    gp_prim q = *p;
+    write_meta(q, &meta[w * sc.P + ag], sc);
+}
+
+// ---- O_vec -------------------------------------------------------------------------------------------------------
+constexpr int kObsWarps = 8;                      // agents per CTA (one warp each), all of the same world
+constexpr unsigned long long kObsNone = 0xFFFFFFFFFFFFFFFFull;
+
+struct ObsArgs {
+    int groups_per_world, K, M, nwarps;
+    float r2;                                     // radius * radius (one fp32 product, formed on the host: O1)
+    const float4 *state;                          // [Wn][A][2]; speed = .x of the first
+    int32_t *agent_idx; float *agent_feat; int32_t *road_idx; float *road_feat;
+};
+
+// K (or M) rounds of "take the smallest remaining key": lanes scan the warp's key array in shared memory, a warp
+// minimum picks the winner, its slot is struck out.  Keys are d2 bits << 32 | index (d2 >= 0: unsigned order = fp32
+// order, ties by index: contract O1).  sel[r] = index taken in round r or -1.
+__device__ __forceinline__ void obs_select(unsigned long long *keys, int n, int rounds, int idx_base, int *sel, int lane) {
+    for (int r = 0; r < rounds; ++r) {
+        unsigned long long best = kObsNone;
+        for (int q = lane; q < n; q += 32) best = min(best, keys[q]);
+#pragma unroll
+        for (int o = 16; o; o >>= 1) best = min(best, __shfl_xor_sync(0xffffffffu, best, o));
+        const int idx = best == kObsNone ? -1 : (int)(uint32_t)best;
+        if (lane == 0) {
+            sel[r] = idx;
+            if (idx >= 0) keys[idx - idx_base] = kObsNone;
+        }
+        __syncwarp();
+    }
+}
+
+// Grid: one CTA per (world, group of nwarps agents).  Dynamic shared memory: float4 s_a[P] (x, y, cos, sin),
+// float4 s_b[P] (2 hx, 2 hy, speed | cls, road flag), unsigned long long s_keys[nwarps][max(A, Q)], int s_sel[nwarps][max(K, M)].
+__global__ void __launch_bounds__(kObsWarps * 32)
+k_observe_vec(SceneConst sc, ObsArgs oa, const gp_prim *__restrict__ prims) {
+    extern __shared__ __align__(16) unsigned char smem[];
+    const int P = sc.P, A = sc.A, Q = sc.Q;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int nmax = max(A, Q), rmax = max(oa.K, oa.M);
+    float4 *s_a = reinterpret_cast<float4 *>(smem);
+    float4 *s_b = s_a + P;
+    unsigned long long *s_keys = reinterpret_cast<unsigned long long *>(s_b + P) + (size_t)warp * nmax;
+    int *s_sel = reinterpret_cast<int *>(reinterpret_cast<unsigned long long *>(s_b + P) + (size_t)oa.nwarps * nmax) + warp * rmax;
+    const int w = blockIdx.x / oa.groups_per_world;
+    const int i = (blockIdx.x - w * oa.groups_per_world) * oa.nwarps + warp;       // agent
+    const gp_prim *wp = prims + (size_t)w * P;
+    for (int k = threadIdx.x; k < P; k += blockDim.x) {
+        const float4 *rec = reinterpret_cast<const float4 *>(&wp[k]);
+        const float4 p0 = __ldg(rec), p1 = __ldg(rec + 1), p2 = __ldg(rec + 2);    // cx cy cz hx | hy hz ck sk | cls inst shape pad
+        s_a[k] = make_float4(p0.x, p0.y, p1.z, p1.w);
+        const bool road = k >= A && __float_as_int(p2.z) == GP_SHAPE_BOX && p1.y == 0.0f;     // flat strips only
+        const float third = k < A ? __ldg(&oa.state[2 * ((size_t)w * A + k)]).x : (float)__float_as_int(p2.x);
+        s_b[k] = make_float4(c_mul(2.0f, p0.w), c_mul(2.0f, p1.x), third, road ? 1.0f : 0.0f);
+    }
+    __syncthreads();
+    if (i >= A) return;
+    const float4 e = s_a[i];
+    const float ev = s_b[i].z;
+    const size_t ai = (size_t)w * A + i;
+    // ---- surrounding agents -----------------------------------------------------------------------
+    if (oa.K > 0) {
+        for (int j = lane; j < A; j += 32) {
+            const float4 q = s_a[j];
+            const float dx = c_sub(q.x, e.x), dy = c_sub(q.y, e.y);
+            const float d2 = c_fma(dy, dy, c_mul(dx, dx));                                      // O1
+            s_keys[j] = (j != i && d2 <= oa.r2) ? ((unsigned long long)__float_as_uint(d2) << 32) | (uint32_t)j : kObsNone;
+        }
+        __syncwarp();
+        obs_select(s_keys, A, oa.K, 0, s_sel, lane);
+        for (int r = lane; r < oa.K; r += 32) {
+            const int j = s_sel[r];
+            float4 f0 = make_float4(0.f, 0.f, 0.f, 0.f), f1 = f0;
+            if (j >= 0) {
+                const float4 q = s_a[j], b = s_b[j];
+                const float dx = c_sub(q.x, e.x), dy = c_sub(q.y, e.y);
+                f0 = make_float4(c_fma(e.w, dy, c_mul(e.z, dx)), c_fma(e.z, dy, -c_mul(e.w, dx)), b.x, b.y);        // O2
+                f1 = make_float4(c_fma(e.w, q.w, c_mul(e.z, q.z)), c_fma(e.z, q.w, -c_mul(e.w, q.z)), c_sub(b.z, ev), 1.0f);   // O3
+            }
+            oa.agent_idx[ai * oa.K + r] = j;
+            float4 *o = reinterpret_cast<float4 *>(oa.agent_feat + (ai * oa.K + r) * 8);
+            o[0] = f0; o[1] = f1;
+        }
+        __syncwarp();
+    }
+    // ---- road segments ----------------------------------------------------------------------------
+    if (oa.M > 0) {
+        for (int k = lane; k < Q; k += 32) {
+            const float4 q = s_a[A + k];
+            const float dx = c_sub(q.x, e.x), dy = c_sub(q.y, e.y);
+            const float d2 = c_fma(dy, dy, c_mul(dx, dx));
+            s_keys[k] = (s_b[A + k].w != 0.0f && d2 <= oa.r2) ? ((unsigned long long)__float_as_uint(d2) << 32) | (uint32_t)(A + k) : kObsNone;
+        }
+        __syncwarp();
+        obs_select(s_keys, Q, oa.M, A, s_sel, lane);
+        for (int r = lane; r < oa.M; r += 32) {
+            const int k = s_sel[r];
+            float4 f0 = make_float4(0.f, 0.f, 0.f, 0.f), f1 = f0;
+            if (k >= 0) {
+                const float4 q = s_a[k], b = s_b[k];
+                const float dx = c_sub(q.x, e.x), dy = c_sub(q.y, e.y);
+                f0 = make_float4(c_fma(e.w, dy, c_mul(e.z, dx)), c_fma(e.z, dy, -c_mul(e.w, dx)), b.x,
+                                 c_fma(e.w, q.w, c_mul(e.z, q.z)));
+                f1 = make_float4(c_fma(e.z, q.w, -c_mul(e.w, q.z)), b.z, 1.0f, 0.0f);
+            }
+            oa.road_idx[ai * oa.M + r] = k;
+            float4 *o = reinterpret_cast<float4 *>(oa.road_feat + (ai * oa.M + r) * 8);
+            o[0] = f0; o[1] = f1;
+        }
+    }
+}
+
+}  // namespace gp

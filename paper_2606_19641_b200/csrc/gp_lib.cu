@@ -11,6 +11,7 @@
 #include "gp_kernel_cull.cuh"
 #include "gp_kernel_render.cuh"
 #include "gp_kernel_raster.cuh"
+#include "gp_kernel_sim.cuh"
 
 using namespace gp;
 
@@ -39,7 +40,8 @@ struct gp_ctx {
     std::vector<Timed> timed;                                    // GP_OPT_TIMING records
     std::vector<cudaEvent_t> ev_pool;
     uint64_t launches = 0;
-    unsigned timing_seq[4] = {0, 0, 0, 0};
+    unsigned timing_seq[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    size_t obs_smem_set = 0;
     size_t render_smem_set = 0, raster_smem_set = 0;
     // gp_render_batch_host staging
     float *d_pose = nullptr;
@@ -64,7 +66,7 @@ struct LaunchTimer {
         cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;              // no event records inside a graph capture
         if (cudaStreamIsCapturing(s, &cap) != cudaSuccess) { cudaGetLastError(); return; }
         if (cap != cudaStreamCaptureStatusNone) return;
-        on = (c->timing_seq[kernel & 3]++ % (unsigned)c->opt_timing) == 0;     // every opt_timing-th launch of this kernel
+        on = (c->timing_seq[kernel & 7]++ % (unsigned)c->opt_timing) == 0;     // every opt_timing-th launch of this kernel
         if (!on) return;
         if (c->timed.size() >= kMaxTimed) {                                     // never polled: recycle the oldest record
             c->ev_pool.push_back(c->timed.front().a); c->ev_pool.push_back(c->timed.front().b);
@@ -270,6 +272,61 @@ extern "C" int gp_agents_update(gp_ctx *c, const float *d_pose, void *stream_) {
         LaunchTimer lt(c, GP_KERNEL_UPDATE, static_cast<cudaStream_t>(stream_));
         k_agents_update<<<(unsigned)((n + 255) / 256), 256, 0, static_cast<cudaStream_t>(stream_)>>>(
             c->sc, reinterpret_cast<const float4 *>(d_pose), c->d_prims, c->d_meta);
+    }
+    c->launches += 1;
+    CK(cudaGetLastError());
+    return GP_OK;
+}
+
+extern "C" int gp_dynamics_step(gp_ctx *c, const gp_dyn_params *par, const int32_t *d_action, float *d_state,
+                                float *d_pose, void *stream_) {
+    if (!c || !par || !d_action || !d_state || !d_pose) return GP_ERR_ARG;
+    if (!c->have_scene) return GP_ERR_STATE;
+    if (!(par->dt > 0.0f) || !(par->a_lon_max >= 0.0f) || !(par->a_lat_max >= 0.0f) || !(par->v_max >= 0.0f) ||
+        !(par->steer_max >= 0.0f) || !(par->steer_rate_max >= 0.0f) || !(par->v_eps > 0.0f) || !(par->extent >= 0.0f))
+        return GP_ERR_ARG;
+    if (!aligned16(d_state) || !aligned16(d_pose)) return GP_ERR_ALIGN;
+    GP_ON_DEVICE(c);
+    const size_t n = (size_t)c->sc.Wn * c->sc.A;
+    {
+        LaunchTimer lt(c, GP_KERNEL_DYNAMICS, static_cast<cudaStream_t>(stream_));
+        k_dynamics_step<<<(unsigned)((n + 127) / 128), 128, 0, static_cast<cudaStream_t>(stream_)>>>(
+            c->sc, *par, d_action, reinterpret_cast<float4 *>(d_state), reinterpret_cast<float4 *>(d_pose), c->d_prims, c->d_meta);
+    }
+    c->launches += 1;
+    CK(cudaGetLastError());
+    return GP_OK;
+}
+
+extern "C" int gp_observe_vec(gp_ctx *c, const float *d_state, int K, int M, float radius, int32_t *d_agent_idx,
+                              float *d_agent_feat, int32_t *d_road_idx, float *d_road_feat, void *stream_) {
+    if (!c || !d_state || K < 0 || M < 0 || K > 1024 || M > 1024 || (K == 0 && M == 0) || !(radius >= 0.0f)) return GP_ERR_ARG;
+    if ((K > 0 && (!d_agent_idx || !d_agent_feat)) || (M > 0 && (!d_road_idx || !d_road_feat))) return GP_ERR_ARG;
+    if (!c->have_scene) return GP_ERR_STATE;
+    if (!aligned16(d_state) || !aligned16(d_agent_feat) || !aligned16(d_road_feat)) return GP_ERR_ALIGN;
+    GP_ON_DEVICE(c);
+    const SceneConst &sc = c->sc;
+    ObsArgs oa;
+    oa.K = K; oa.M = M; oa.r2 = radius * radius;
+    oa.state = reinterpret_cast<const float4 *>(d_state);
+    oa.agent_idx = d_agent_idx; oa.agent_feat = d_agent_feat; oa.road_idx = d_road_idx; oa.road_feat = d_road_feat;
+    // agents per CTA: as many warps (<= kObsWarps) as leave the world's records + per-warp key arrays within shared memory
+    const size_t nmax = (size_t)std::max(sc.A, sc.Q), rmax = (size_t)std::max(K, M);
+    int nw = std::min(kObsWarps, sc.A);
+    size_t smem = 0;
+    for (;; --nw) {
+        smem = (size_t)sc.P * 32 + (size_t)nw * nmax * 8 + (size_t)nw * rmax * 4;
+        if (smem <= 200 * 1024 || nw == 1) break;
+    }
+    if (smem > 200 * 1024) return GP_ERR_ARG;
+    oa.nwarps = nw; oa.groups_per_world = (sc.A + nw - 1) / nw;
+    if (smem > c->obs_smem_set) {
+        CK(cudaFuncSetAttribute(k_observe_vec, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        c->obs_smem_set = smem;
+    }
+    {
+        LaunchTimer lt(c, GP_KERNEL_OBSERVE, static_cast<cudaStream_t>(stream_));
+        k_observe_vec<<<(unsigned)((size_t)sc.Wn * oa.groups_per_world), nw * 32, smem, static_cast<cudaStream_t>(stream_)>>>(sc, oa, c->d_prims);
     }
     c->launches += 1;
     CK(cudaGetLastError());

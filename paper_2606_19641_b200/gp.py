@@ -18,13 +18,13 @@ GP_OK, GP_ERR_ARG, GP_ERR_ALIGN, GP_ERR_STATE, GP_ERR_RANGE, GP_ERR_CUDA, GP_ERR
 GP_OPT_PATH, GP_OPT_STATS, GP_OPT_TIMING, GP_OPT_STAGE_CAP, GP_OPT_STRIP_PX, GP_OPT_GATHER, GP_OPT_SPHERES = 1, 2, 3, 4, 5, 6, 7
 GP_OPT_VARIANT, GP_OPT_TILE_PX, GP_OPT_PIPELINE = 8, 9, 10
 GP_VARIANT_RAY, GP_VARIANT_RASTER = 0, 1
-GP_KERNEL_UPDATE, GP_KERNEL_CULL, GP_KERNEL_RENDER, GP_KERNEL_BRUTE = 0, 1, 2, 3
+GP_KERNEL_UPDATE, GP_KERNEL_CULL, GP_KERNEL_RENDER, GP_KERNEL_BRUTE, GP_KERNEL_DYNAMICS, GP_KERNEL_OBSERVE = 0, 1, 2, 3, 4, 5
 GP_PATH_FAST, GP_PATH_BRUTE = 0, 1
 
 EXPORTS = ("gp_create", "gp_destroy", "gp_set_option", "gp_scene_upload", "gp_agents_update",
            "gp_cameras_set", "gp_render_batch", "gp_render_batch_host", "gp_stats", "gp_kernel_time",
            "gp_launch_count", "gp_camera_rig_set", "gp_statics_from_polylines", "gp_statics_update",
-           "gp_error_string")
+           "gp_dynamics_step", "gp_observe_vec", "gp_error_string")
 
 
 class SceneDesc(ctypes.Structure):
@@ -32,6 +32,12 @@ class SceneDesc(ctypes.Structure):
                 ("quads_per_world", ctypes.c_int32), ("cam_height", ctypes.c_float),
                 ("t_max", ctypes.c_float), ("light", ctypes.c_float * 3), ("ambient", ctypes.c_float),
                 ("palette", (ctypes.c_uint8 * 3) * 8)]
+
+
+class DynParams(ctypes.Structure):
+    _fields_ = [("dt", ctypes.c_float), ("a_lon_max", ctypes.c_float), ("a_lat_max", ctypes.c_float),
+                ("v_max", ctypes.c_float), ("steer_max", ctypes.c_float), ("steer_rate_max", ctypes.c_float),
+                ("v_eps", ctypes.c_float), ("extent", ctypes.c_float)]
 
 
 class Camera(ctypes.Structure):
@@ -75,6 +81,8 @@ def lib():
         L.gp_camera_rig_set.argtypes = [vp, ci, vp]
         L.gp_statics_update.argtypes = [vp, vp, ci, ci, vp]
         L.gp_statics_from_polylines.argtypes = [vp, vp, ci, ci, cf, cf, ci, ci, vp]
+        L.gp_dynamics_step.argtypes = [vp, ctypes.POINTER(DynParams), vp, vp, vp, vp]
+        L.gp_observe_vec.argtypes = [vp, vp, ci, ci, cf, vp, vp, vp, vp, vp]
         L.gp_error_string.argtypes = [ci]
         L.gp_error_string.restype = ctypes.c_char_p
         for name in EXPORTS[:-1]:
@@ -159,6 +167,22 @@ class Renderer:
         assert d_points.dim() == 4 and d_points.shape[3] == 2 and d_points.is_contiguous()
         _check(lib().gp_statics_from_polylines(self._h, _dptr(d_points), int(d_points.shape[1]), int(d_points.shape[2]),
                                                float(half_width), float(z), int(cls), int(q_begin), _stream(self.device)))
+
+    def dynamics_step(self, params, d_action, d_state, d_pose):
+        """params: dict or DynParams; d_action CUDA int32 [Wn][A]; d_state CUDA float32 [Wn][A][8] and d_pose CUDA
+        float32 [Wn][A][4], both updated in place; the scene's agent records follow the new poses."""
+        if not isinstance(params, DynParams):
+            q = DynParams()
+            for k, v in dict(params).items():
+                setattr(q, k, float(v))
+            params = q
+        _check(lib().gp_dynamics_step(self._h, ctypes.byref(params), _dptr(d_action), _dptr(d_state), _dptr(d_pose),
+                                      _stream(self.device)))
+
+    def observe_vec(self, d_state, K, M, radius, d_agent_idx, d_agent_feat, d_road_idx, d_road_feat):
+        """O_vec into caller-owned CUDA tensors: int32 [Wn][A][K], float32 [Wn][A][K][8], int32 [Wn][A][M], float32 [Wn][A][M][8]."""
+        _check(lib().gp_observe_vec(self._h, _dptr(d_state), int(K), int(M), float(radius), _dptr(d_agent_idx),
+                                    _dptr(d_agent_feat), _dptr(d_road_idx), _dptr(d_road_feat), _stream(self.device)))
 
     def camera_rig_set(self, rig):
         """rig: array-like [C][>=3] = (cos yaw offset, sin yaw offset, mount) per camera of every agent."""
