@@ -54,6 +54,7 @@ def parse():
                     help="capture each step (pose update + cull + render) in a CUDA graph and time the replays")
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-sim", action="store_true", help="skip the dynamics + O_vec + render leg (agent steps / s)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
 
@@ -310,6 +311,78 @@ def run_b200(args):
     step(n_frames - 1, stats)
     r.set_option(gp.GP_OPT_STATS, 0)
 
+    # calibration probes: write-only bandwidth with the render pass's store pattern over the same output
+    # planes, and the FP32 FMA rate at the clock this GPU runs it at; after the timed region, never inside it
+    probes = None
+    try:
+        n_probe = (min(cfg.views, chunk * vpw) * cfg.H * cfg.W) // 128 * 128
+        st_best, st_med = r.probe(gp.GP_PROBE_STORE, n_probe, 10, outs)
+        fma_best, fma_med = r.probe(gp.GP_PROBE_FMA, 0, 10)
+        probes = {"store_gbs_best": st_best, "store_gbs_median": st_med, "store_bytes": n_probe * 12,
+                  "fma_tflops_best": fma_best, "fma_tflops_median": fma_med,
+                  "how": "gp_probe: 10 launches after 1 warm-up each, CUDA events; store = 12 B/px plane pattern of k_render over "
+                         "the bench's own output planes; fma = 8 FFMA chains/thread, 148x8 CTAs x 256 threads"}
+    except Exception as ex:  # noqa: BLE001
+        probes = {"error": repr(ex)[:200]}
+
+    # the whole simulator step on the device: jerk-bicycle dynamics fused
+    # with the pose update -> O_vec (nearest 16 agents, nearest 32 road segments within 100 m) -> cull -> render, no
+    # host transfer; actions are resident in HBM.  Not the headline metric: reported beside it as agent steps / s.
+    agent_step = None
+    if not args.no_sim:
+        try:
+            K_OBS, M_OBS, RADIUS = 16, 32, 100.0
+            sim_steps = min(args.steps, 50)
+            gen = torch.Generator(device=dev); gen.manual_seed(1234 + rank)
+            actions = torch.randint(0, 12, (sim_steps + 3, cfg.n_worlds, cfg.agents), dtype=torch.int32, device=dev, generator=gen)
+            psi = np.arctan2(agents["sin_yaw"].astype(np.float64), agents["cos_yaw"].astype(np.float64))
+            st0 = np.zeros((cfg.n_worlds, cfg.agents, 8), np.float32)
+            st0[..., 0] = speed                                  # the generator's per-agent speed
+            st0[..., 4] = psi
+            d_state = torch.from_numpy(st0).to(dev)
+            d_sp = torch.from_numpy(poses[0].copy()).to(dev)
+            obs = (torch.empty((cfg.n_worlds, cfg.agents, K_OBS), dtype=torch.int32, device=dev),
+                   torch.empty((cfg.n_worlds, cfg.agents, K_OBS, 8), dtype=torch.float32, device=dev),
+                   torch.empty((cfg.n_worlds, cfg.agents, M_OBS), dtype=torch.int32, device=dev),
+                   torch.empty((cfg.n_worlds, cfg.agents, M_OBS, 8), dtype=torch.float32, device=dev))
+            dyn = gp.DynParams(0.1, 6.0, 4.0, 20.0, 0.6, 0.8, 0.5, float(cfg.extent))
+
+            def sim_step(i):
+                r.dynamics_step(dyn, actions[i], d_state, d_sp)
+                r.observe_vec(d_state, K_OBS, M_OBS, RADIUS, *obs)
+                for w_begin, nw in chunks:
+                    r.render_batch(w_begin, nw, cfg.H, cfg.W, fov, *subs[nw])
+
+            for i in range(3):
+                sim_step(i)
+            r.set_option(gp.GP_OPT_TIMING, 4 if sim_steps >= 16 else 1)
+            kids = (("dynamics", gp.GP_KERNEL_DYNAMICS), ("observe", gp.GP_KERNEL_OBSERVE), ("cull", gp.GP_KERNEL_CULL),
+                    ("render", gp.GP_KERNEL_RENDER))
+            for _, k in kids:
+                r.kernel_time(k)
+            l0 = r.launch_count()
+            barrier()
+            ev0.record()
+            for i in range(3, 3 + sim_steps):
+                sim_step(i)
+            ev1.record()
+            barrier()
+            sim_ms = shard.max_over_ranks(ev0.elapsed_time(ev1), dev)
+            kt = {name: r.kernel_time(k) for name, k in kids}
+            r.set_option(gp.GP_OPT_TIMING, 0)
+            n_s = max(1, kt["dynamics"][1])
+            agent_step = {"value": world_size * cfg.n_worlds * cfg.agents * sim_steps / (sim_ms * 1e-3), "unit": "agent steps/s",
+                          "ms_per_step": sim_ms / sim_steps, "steps": sim_steps,
+                          "views_per_s": world_size * cfg.views * sim_steps / (sim_ms * 1e-3),
+                          "kernels_ms_per_step": {k: v[0] / n_s for k, v in kt.items()},
+                          "gpu_launches": int(r.launch_count() - l0),
+                          "what": "gp_dynamics_step (12 random actions, dt 0.1 s, torus %g m) + gp_observe_vec (K=%d agents, M=%d road "
+                                  "segments, %g m) + gp_render_batch, all on the device" % (cfg.extent, K_OBS, M_OBS, RADIUS),
+                          "context": "PAPER.md:8 quotes ~50k agent steps/s on 1 GPU for its simulator with rendering (other hardware, "
+                                     "nuPlan scenes, resolution unstated): context, not a like-for-like baseline"}
+        except Exception as ex:  # noqa: BLE001 - report, do not hide
+            agent_step = {"value": None, "unit": "agent steps/s", "error": repr(ex)[:300]}
+
     # end to end through the host-buffer entry point (pinned host memory, copies inside the timed region)
     e2e = None
     if not args.no_e2e:
@@ -358,15 +431,22 @@ def run_b200(args):
     render_launches_per_step = max(1.0, r_n / steps_sampled)   # render calls x pipeline chunks per call (GP_OPT_PIPELINE)
     alg_bytes_launch = alg_bytes / render_launches_per_step    # one render launch = one world chunk of the pipeline
     achieved = alg_bytes_launch / (r_avg_ms * 1e-3) / 1e9
-    traffic = None
-    tpath = os.path.join(ROOT, "profiles", "r01_traffic.txt")      # from the committed ncu --set full capture
-    if os.path.exists(tpath) and not args.worlds and not args.res and not args.hw:
-        for line in open(tpath):
-            part = line.split()
-            if len(part) == 2 and part[0] == cfg.name:
-                traffic = int(part[1])
+    # dram bytes of one k_render launch from a COMMITTED ncu --set full capture of this command (not measured live:
+    # a run under the profiler is never a bench run); the file names its source captures
+    traffic, traffic_source = None, None
+    for tname in ("r02_traffic.txt", "r01_traffic.txt"):
+        tpath = os.path.join(ROOT, "profiles", tname)
+        if traffic is None and os.path.exists(tpath) and not args.worlds and not args.hw:
+            for line in open(tpath):
+                part = line.split()
+                if len(part) >= 2 and part[0] == (cfg.name if not args.res else "%s%d" % (cfg.name, args.res)):
+                    traffic = int(part[1])
+                    traffic_source = "profiles/%s (dram__bytes_read.sum + dram__bytes_write.sum of one k_render launch, earlier " \
+                                     "ncu --set full capture; see profiles/r02_render_cull_full.md)" % tname
     sm_mhz = (clocks or {}).get("sm_mhz") or 1965.0
-    fp32_peak = 148 * 128 * 2 * sm_mhz * 1e6
+    fp32_nominal = 148 * 128 * 2 * sm_mhz * 1e6
+    fp32_peak = (probes or {}).get("fma_tflops_best", 0) * 1e12 or fp32_nominal
+    wr_peak = (probes or {}).get("store_gbs_best")
     t_fp32_ms = stats["executed_tests"] * FP32_OPS_PER_TEST / fp32_peak * 1e3
     t_hbm_ms = alg_bytes / (peak * 1e9) * 1e3
     step_ms = ms / args.steps
@@ -382,15 +462,23 @@ def run_b200(args):
         "kernel_samples": {k: int(v[1]) for k, v in ktimes.items()},
         "cuda_graph": bool(graphs),
         "roofline": {"bound": "hbm", "kernel": "k_render", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                     "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
+                     "frac": achieved / peak, "traffic": traffic, "traffic_source": traffic_source, "peak_source": peak_src,
+                     "peak_write_only": wr_peak, "frac_write_only": (achieved / wr_peak) if wr_peak else None,
+                     "peak_write_only_source": "gp_probe(GP_PROBE_STORE) in this run: write-only kernel with k_render's store pattern",
                      "algorithmic_bytes_per_launch": alg_bytes_launch, "avg_launch_ms": r_avg_ms,
                      "launches_per_step": render_launches_per_step, "share_of_step": r_ms / steps_sampled / step_ms,
                      "note": "the culls of later world chunks run concurrently with these launches on a second stream"},
         "roofline_step": {"t_hbm_ms": t_hbm_ms, "t_fp32_ms": t_fp32_ms, "frac_of_slower_roof": max(t_hbm_ms, t_fp32_ms) / step_ms,
                           "executed_tests": stats["executed_tests"], "listed_pairs": stats["listed_pairs"],
+                          "frac_of_write_only_roof": (alg_bytes / (wr_peak * 1e9) * 1e3 / step_ms) if wr_peak else None,
                           "tests_per_pixel": stats["executed_tests"] / npx, "fp32_peak_tflops": fp32_peak / 1e12,
+                          "fp32_peak_source": "gp_probe(GP_PROBE_FMA) in this run" if (probes or {}).get("fma_tflops_best") else
+                                              "nominal 148 SM x 128 lanes x 2 x sampled SM clock",
+                          "fp32_nominal_tflops": fp32_nominal / 1e12,
                           "fp32_ops_per_test": FP32_OPS_PER_TEST},
         "e2e": e2e,
+        "agent_step": agent_step,
+        "probes": probes,
     }
     if not args.no_cpu_baseline and world_size == 1:
         threads = max(1, min(64, os.cpu_count() or 1))
@@ -400,6 +488,8 @@ def run_b200(args):
         n1 = max(1, min(cfg.views, int(round(1.5 / per_core_s))))
         sec1 = oracle_sample(cfg, n1, 1)
         out["cpu_baseline"] = {"value": n_views / sec, "unit": UNIT, "cores": threads, "kind": "oracle",
+                               "note": "the oracle is the plain definition: every primitive of the world per pixel, scalar C, no culling; "
+                                       "a reported baseline, not a tuned CPU renderer",
                                "one_core": {"value": n1 / sec1, "unit": UNIT, "sample": "%d views, 1 thread, %.1f s" % (n1, sec1)},
                                "sample": "%d views of the workload (frame 0), all-primitive fp32 oracle (oracle/gp_oracle.c), %d threads, %.1f s"
                                          % (n_views, threads, sec)}

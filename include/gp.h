@@ -23,6 +23,7 @@
 #ifndef GP_H_
 #define GP_H_
 
+#include <stddef.h>
 #include <stdint.h>
 
 #ifdef __cplusplus
@@ -246,6 +247,18 @@ int gp_dynamics_step(gp_ctx *ctx, const gp_dyn_params *params, const int32_t *d_
  * Feature pointers 16-byte aligned. */
 int gp_observe_vec(gp_ctx *ctx, const float *d_state, int K, int M, float radius, int32_t *d_agent_idx,
                    float *d_agent_feat, int32_t *d_road_idx, float *d_road_feat, void *stream);
+
+/* Calibration probes for the roofline denominators; synchronises `stream`.
+ *   GP_PROBE_STORE: a write-only kernel with the render pass's exact store pattern (per 128 pixels: 4-byte stores to the
+ *     class plane and the three colour planes, 16-byte stores to the instance and depth planes = 12 B / pixel) over
+ *     n_pixels pixels (a multiple of 128) of the caller's DEVICE planes (sized as for gp_render_batch with n_pixels
+ *     pixels in all; their content is overwritten).  Result: GB/s.
+ *   GP_PROBE_FMA: 8 independent FFMA chains per thread on 148 x 8 CTAs x 256 threads, no memory traffic; the plane
+ *     pointers and n_pixels are ignored.  Result: TFLOP/s (2 flop per FFMA) at the clock the GPU runs this at.
+ * Runs `iters` timed launches after one warm-up; *best = highest rate, *median (may be NULL) = the median. */
+enum { GP_PROBE_STORE = 0, GP_PROBE_FMA = 1 };
+int gp_probe(gp_ctx *ctx, int kind, size_t n_pixels, int iters, uint8_t *d_class, int32_t *d_instance, float *d_depth,
+             uint8_t *d_rgb, void *stream, double *best, double *median);
 
 /* Counters of the last gp_render_batch issued with GP_OPT_STATS = 1 (synchronises the device):
  * executed_tests = ray/primitive slab tests actually evaluated, listed_pairs = (view, primitive)

@@ -1,0 +1,48 @@
+// gp_kernel_probe.cuh — calibration probes for the roofline denominators ("a tracked write-only HBM
+// bandwidth and an FP32 FMA peak measured under this kernel's clock").  Not part of the render path.
+#pragma once
+#include "gp_device.cuh"
+
+namespace gp {
+
+// Write-only stream with the render pass's exact store pattern: per 128-pixel group a warp writes one 4-byte store per
+// lane to the class plane and to each of the three colour planes, and one 16-byte store per lane to the instance and
+// depth planes (12 bytes per pixel, full 128-byte lines).  Groups are dealt to CTAs in ascending order, 16 per CTA.
+__global__ void __launch_bounds__(128, 8)
+k_probe_store(size_t n_groups, uint8_t *o_cls, int32_t *o_inst, float *o_depth, uint8_t *o_rgb, size_t rgb_plane, uint32_t val) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const size_t g0 = (size_t)blockIdx.x * 16;
+    for (int q = warp; q < 16; q += 4) {
+        const size_t g = g0 + q;
+        if (g >= n_groups) return;
+        const size_t o = g * 128 + lane * 4;
+        *reinterpret_cast<uint32_t *>(o_cls + o) = val;
+        *reinterpret_cast<int4 *>(o_inst + o) = make_int4(-1, -1, -1, -1);
+        *reinterpret_cast<float4 *>(o_depth + o) = make_float4(1.0f, 1.0f, 1.0f, 1.0f);
+        // rgb is [view][3][HW]: the probe treats the whole buffer as one "view" of n pixels
+        *reinterpret_cast<uint32_t *>(o_rgb + o) = val;
+        *reinterpret_cast<uint32_t *>(o_rgb + rgb_plane + o) = val;
+        *reinterpret_cast<uint32_t *>(o_rgb + 2 * rgb_plane + o) = val;
+    }
+}
+
+// FP32 FMA throughput: 8 independent dependent-chains of FFMA per thread, no memory traffic; out is written only if a
+// result is NaN (never), which keeps the chains alive.
+__global__ void __launch_bounds__(256)
+k_probe_fma(int iters, float seed, float *out) {
+    float a0 = seed, a1 = seed + 1.0f, a2 = seed + 2.0f, a3 = seed + 3.0f, a4 = seed + 4.0f, a5 = seed + 5.0f, a6 = seed + 6.0f,
+          a7 = seed + 7.0f;
+    const float m = 0.999f, c = 0.001f * (float)(threadIdx.x & 7);
+#pragma unroll 1
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int u = 0; u < 16; ++u) {
+            a0 = fmaf(a0, m, c); a1 = fmaf(a1, m, c); a2 = fmaf(a2, m, c); a3 = fmaf(a3, m, c);
+            a4 = fmaf(a4, m, c); a5 = fmaf(a5, m, c); a6 = fmaf(a6, m, c); a7 = fmaf(a7, m, c);
+        }
+    }
+    const float s = ((a0 + a1) + (a2 + a3)) + ((a4 + a5) + (a6 + a7));
+    if (s != s) out[0] = s;
+}
+
+}  // namespace gp

@@ -1,5 +1,6 @@
 // gp_lib.cu — the C ABI of include/gp.h on top of the sm_100a kernels.  Host logic only: argument
 // validation, device residency of the scene, scratch sizing, launches.  No CPU rendering path exists.
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -12,6 +13,7 @@
 #include "gp_kernel_render.cuh"
 #include "gp_kernel_raster.cuh"
 #include "gp_kernel_sim.cuh"
+#include "gp_kernel_probe.cuh"
 
 using namespace gp;
 
@@ -736,6 +738,45 @@ extern "C" int gp_render_batch_host(gp_ctx *c, const float *h_pose, int world_be
     }
     CK(cudaStreamSynchronize(c->copy_stream));
     CK(cudaStreamSynchronize(stream));
+    return GP_OK;
+}
+
+extern "C" int gp_probe(gp_ctx *c, int kind, size_t n_pixels, int iters, uint8_t *d_class, int32_t *d_instance,
+                        float *d_depth, uint8_t *d_rgb, void *stream_, double *best, double *median) {
+    if (!c || !best || iters < 1 || iters > 1000) return GP_ERR_ARG;
+    GP_ON_DEVICE(c);
+    cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+    cudaEvent_t e0, e1;
+    CK(cudaEventCreate(&e0)); CK(cudaEventCreate(&e1));
+    std::vector<double> rate;
+    int rc = GP_OK;
+    for (int it = 0; it < iters + 1 && rc == GP_OK; ++it) {                 // the first launch is a warm-up
+        cudaEventRecord(e0, stream);
+        double units = 0.0;
+        if (kind == GP_PROBE_STORE) {
+            if (!d_class || !d_instance || !d_depth || !d_rgb || n_pixels < 128 || (n_pixels & 127)) { rc = GP_ERR_ARG; break; }
+            if (!aligned16(d_class) || !aligned16(d_instance) || !aligned16(d_depth) || !aligned16(d_rgb)) { rc = GP_ERR_ALIGN; break; }
+            const size_t groups = n_pixels / 128;
+            k_probe_store<<<(unsigned)((groups + 15) / 16), 128, 0, stream>>>(groups, d_class, d_instance, d_depth, d_rgb,
+                                                                                n_pixels, 0x01010101u * (uint32_t)(it & 3));
+            units = (double)n_pixels * 12.0 / 1e9;                              // GB
+        } else if (kind == GP_PROBE_FMA) {
+            const int reps = 4096;
+            k_probe_fma<<<148 * 8, 256, 0, stream>>>(reps, 1.0f + (float)it, reinterpret_cast<float *>(c->d_stats));
+            units = 2.0 * 148.0 * 8 * 256 * (double)reps * 16 * 8 / 1e12;       // TFLOP
+        } else { rc = GP_ERR_ARG; break; }
+        c->launches += 1;
+        cudaEventRecord(e1, stream);
+        if (cudaEventSynchronize(e1) != cudaSuccess || cudaGetLastError() != cudaSuccess) { rc = cuda_fail(cudaGetLastError(), "gp_probe"); break; }
+        float ms = 0.0f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        if (it > 0) rate.push_back(units / (ms * 1e-3));
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    if (rc != GP_OK) return rc;
+    std::sort(rate.begin(), rate.end());
+    *best = rate.back();
+    if (median) *median = rate[rate.size() / 2];
     return GP_OK;
 }
 

@@ -20,11 +20,12 @@ GP_OPT_VARIANT, GP_OPT_TILE_PX, GP_OPT_PIPELINE = 8, 9, 10
 GP_VARIANT_RAY, GP_VARIANT_RASTER = 0, 1
 GP_KERNEL_UPDATE, GP_KERNEL_CULL, GP_KERNEL_RENDER, GP_KERNEL_BRUTE, GP_KERNEL_DYNAMICS, GP_KERNEL_OBSERVE = 0, 1, 2, 3, 4, 5
 GP_PATH_FAST, GP_PATH_BRUTE = 0, 1
+GP_PROBE_STORE, GP_PROBE_FMA = 0, 1
 
 EXPORTS = ("gp_create", "gp_destroy", "gp_set_option", "gp_scene_upload", "gp_agents_update",
            "gp_cameras_set", "gp_render_batch", "gp_render_batch_host", "gp_stats", "gp_kernel_time",
            "gp_launch_count", "gp_camera_rig_set", "gp_statics_from_polylines", "gp_statics_update",
-           "gp_dynamics_step", "gp_observe_vec", "gp_error_string")
+           "gp_dynamics_step", "gp_observe_vec", "gp_probe", "gp_error_string")
 
 
 class SceneDesc(ctypes.Structure):
@@ -83,6 +84,8 @@ def lib():
         L.gp_statics_from_polylines.argtypes = [vp, vp, ci, ci, cf, cf, ci, ci, vp]
         L.gp_dynamics_step.argtypes = [vp, ctypes.POINTER(DynParams), vp, vp, vp, vp]
         L.gp_observe_vec.argtypes = [vp, vp, ci, ci, cf, vp, vp, vp, vp, vp]
+        L.gp_probe.argtypes = [vp, ci, ctypes.c_size_t, ci, vp, vp, vp, vp, vp, ctypes.POINTER(ctypes.c_double),
+                               ctypes.POINTER(ctypes.c_double)]
         L.gp_error_string.argtypes = [ci]
         L.gp_error_string.restype = ctypes.c_char_p
         for name in EXPORTS[:-1]:
@@ -183,6 +186,13 @@ class Renderer:
         """O_vec into caller-owned CUDA tensors: int32 [Wn][A][K], float32 [Wn][A][K][8], int32 [Wn][A][M], float32 [Wn][A][M][8]."""
         _check(lib().gp_observe_vec(self._h, _dptr(d_state), int(K), int(M), float(radius), _dptr(d_agent_idx),
                                     _dptr(d_agent_feat), _dptr(d_road_idx), _dptr(d_road_feat), _stream(self.device)))
+
+    def probe(self, kind, n_pixels=0, iters=10, planes=(None, None, None, None)):
+        """(best, median) rate of a calibration probe: GB/s for GP_PROBE_STORE, TFLOP/s for GP_PROBE_FMA."""
+        best, med = ctypes.c_double(), ctypes.c_double()
+        _check(lib().gp_probe(self._h, int(kind), int(n_pixels), int(iters), *[_dptr(t) for t in planes],
+                              _stream(self.device), ctypes.byref(best), ctypes.byref(med)))
+        return best.value, med.value
 
     def camera_rig_set(self, rig):
         """rig: array-like [C][>=3] = (cos yaw offset, sin yaw offset, mount) per camera of every agent."""
