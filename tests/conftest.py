@@ -16,6 +16,21 @@ def pytest_configure(config):
 import gp_scenes as gs  # noqa: E402
 
 
+def pytest_sessionfinish(session, exitstatus):
+    """-m gpu runs: the summed parity counts (pixels compared, excluded tie pixels, how many of those matched anyway,
+    mismatches) go to gpurun_out/parity_report.json, from which profiles/r02_parity.md is written."""
+    try:
+        import json
+        import parity_util
+        if parity_util.REPORT:
+            out = os.path.join(ROOT, "gpurun_out")
+            os.makedirs(out, exist_ok=True)
+            with open(os.path.join(out, "parity_report.json"), "w") as f:
+                json.dump({"exitstatus": int(exitstatus), "report": parity_util.REPORT}, f, indent=1, sort_keys=True)
+    except Exception:       # noqa: BLE001 - reporting must never fail a test run
+        pass
+
+
 def make_prim(cx, cy, cz, hx, hy, hz, cos_yaw=1.0, sin_yaw=0.0, cls=3, inst=0, shape=0):
     p = np.zeros((), dtype=gs.PRIM_DTYPE)
     p["cx"], p["cy"], p["cz"] = cx, cy, cz

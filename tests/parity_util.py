@@ -43,9 +43,21 @@ def oracle_threads():
     return max(1, min(32, (os.cpu_count() or 1)))
 
 
-def compare_views(gpu_planes, view_indices, refs):
+REPORT = {}          # label -> summed compare_views reports; written to gpurun_out/parity_report.json at session end
+
+
+def record(label, rep):
+    acc = REPORT.setdefault(label, {})
+    for k, v in rep.items():
+        acc[k] = acc.get(k, 0) + v
+
+
+def compare_views(gpu_planes, view_indices, refs, label=None):
     """gpu_planes: (cls, inst, depth, rgb) torch tensors; view_indices: indices into them; refs: oracle
-    dicts.  Returns a report dict; raises AssertionError on any violation of the parity rules."""
+    dicts.  Returns a report dict; raises AssertionError on any violation of the parity rules.
+    Rules (BASELINE.json north_star): ids bit-exact except pixels whose two nearest hits lie within 1e-5 m (excluded
+    from the ID and colour comparison only, and counted); depth within 1e-5 relative on EVERY pixel — on an excluded
+    pixel the other of the two near-equal hits may have won, so its tolerance is widened by the 1e-5 m gap."""
     cls, inst, depth, rgb = gpu_planes
     rep = {"pixels": 0, "excluded": 0, "excluded_matched": 0, "id_mismatch": 0, "depth_bad": 0,
            "rgb_mismatch": 0, "depth_bitexact": 0}
@@ -59,15 +71,19 @@ def compare_views(gpu_planes, view_indices, refs):
         rep["excluded"] += int(excl.sum())
         rep["excluded_matched"] += int((ids_ok & excl).sum())
         rep["id_mismatch"] += int((~ids_ok & keep).sum())
-        d_ok = np.abs(g_dep.astype(np.float64) - ref["depth"]) <= DEPTH_RTOL * np.abs(ref["depth"])
-        rep["depth_bad"] += int((~d_ok & keep).sum())
+        d_err = np.abs(g_dep.astype(np.float64) - ref["depth"])
+        d_ok = d_err <= DEPTH_RTOL * np.abs(ref["depth"]) + np.where(excl, TIE_GAP_M, 0.0)
+        rep["depth_bad"] += int((~d_ok).sum())
         rep["depth_bitexact"] += int((g_dep == ref["depth"]).sum())
         if rgb is not None and ref.get("rgb") is not None:
             g_rgb = rgb[vi].cpu().numpy()
             rep["rgb_mismatch"] += int(((g_rgb != ref["rgb"]).any(axis=0) & keep).sum())
+    rep["views"] = len(view_indices)
     assert rep["id_mismatch"] == 0, rep
     assert rep["depth_bad"] == 0, rep
     assert rep["rgb_mismatch"] == 0, rep
+    if label:
+        record(label, rep)
     return rep
 
 
