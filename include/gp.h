@@ -255,8 +255,11 @@ int gp_observe_vec(gp_ctx *ctx, const float *d_state, int K, int M, float radius
  *     pixels in all; their content is overwritten).  Result: GB/s.
  *   GP_PROBE_FMA: 8 independent FFMA chains per thread on 148 x 8 CTAs x 256 threads, no memory traffic; the plane
  *     pointers and n_pixels are ignored.  Result: TFLOP/s (2 flop per FFMA) at the clock the GPU runs this at.
+ *   GP_PROBE_RCP: self-check of the render pass's paired reciprocal (C0: 1.0f / x correctly rounded) against
+ *     __frcp_rn on all 2^32 bit patterns; the plane pointers and n_pixels are ignored.  Result: the number of bit
+ *     patterns whose result differed, summed over the launches (0 = identical).
  * Runs `iters` timed launches after one warm-up; *best = highest rate, *median (may be NULL) = the median. */
-enum { GP_PROBE_STORE = 0, GP_PROBE_FMA = 1 };
+enum { GP_PROBE_STORE = 0, GP_PROBE_FMA = 1, GP_PROBE_RCP = 2 };
 int gp_probe(gp_ctx *ctx, int kind, size_t n_pixels, int iters, uint8_t *d_class, int32_t *d_instance, float *d_depth,
              uint8_t *d_rgb, void *stream, double *best, double *median);
 

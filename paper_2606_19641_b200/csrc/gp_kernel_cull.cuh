@@ -20,7 +20,7 @@ namespace gp {
 constexpr float kNearEps = 0.01f;      // clip plane for the projection bound, metres of planar depth
 constexpr float kNearGuard = 0.05f;    // cross-section this close to the optical centre => whole image
 
-struct PixBounds { float smin, smax, vmin, vmax; };
+struct PixBounds { float smin, smax, vmin, vmax, xmin; };
 
 // 1/x to ~1 ulp in one MUFU instruction (conservative geometry only; never contract arithmetic)
 __device__ __forceinline__ float rcp_fast(float x) {
@@ -29,14 +29,32 @@ __device__ __forceinline__ float rcp_fast(float x) {
     return r;
 }
 
-__device__ __forceinline__ void bound_point(PixBounds &b, float X, float Y, float Z, float E) {
-    // X >= kNearEps.  (Y +- E(1+|s|)) / X bounds the true s for an absolute coordinate error E; the
-    // 1e-6 relative term covers the approximate reciprocal.
-    float inv = rcp_fast(X);
-    float s = Y * inv, v = Z * inv;
-    float ds = fmaf(E * (1.0f + fabsf(s)), inv, 1e-6f * fabsf(s)), dv = fmaf(E * (1.0f + fabsf(v)), inv, 1e-6f * fabsf(v));
+// Projection (s, v) = (Y / X, Z / X) of one camera-frame point with X >= kNearEps, accumulated WITHOUT its error term
+// (fast path); bound_widen() then widens the whole interval once by the largest error any accumulated point can have.
+__device__ __forceinline__ void bound_point(PixBounds &b, float X, float Y, float Z) {
+    const float inv = rcp_fast(X);
+    const float s = Y * inv, v = Z * inv;
+    b.smin = fminf(b.smin, s); b.smax = fmaxf(b.smax, s);
+    b.vmin = fminf(b.vmin, v); b.vmax = fmaxf(b.vmax, v);
+    b.xmin = fminf(b.xmin, X);
+}
+// The same with the point's own error term (precise path: points near the clip plane have large errors that must not
+// be charged to the far end of the primitive).  (Y +- E(1+|s|)) / X bounds the true s for an absolute coordinate error
+// E; the 1e-6 relative term covers the approximate reciprocal.
+__device__ __forceinline__ void bound_point_err(PixBounds &b, float X, float Y, float Z, float E) {
+    const float inv = rcp_fast(X);
+    const float s = Y * inv, v = Z * inv;
+    const float ds = fmaf(E * (1.0f + fabsf(s)), inv, 1e-6f * fabsf(s)), dv = fmaf(E * (1.0f + fabsf(v)), inv, 1e-6f * fabsf(v));
     b.smin = fminf(b.smin, s - ds); b.smax = fmaxf(b.smax, s + ds);
     b.vmin = fminf(b.vmin, v - dv); b.vmax = fmaxf(b.vmax, v + dv);
+}
+// With |s| <= max|s| and X >= xmin over the accumulated points, the one term below is >= every point's own error term,
+// so the widened interval contains each point's own widened interval.  Returns the two widths.
+__device__ __forceinline__ void bound_widen(PixBounds &b, float E, float &ds, float &dv) {
+    const float inv = rcp_fast(b.xmin) * 1.000001f;
+    const float sm = fmaxf(fabsf(b.smin), fabsf(b.smax)), vm = fmaxf(fabsf(b.vmin), fabsf(b.vmax));
+    ds = fmaf(E * (1.0f + sm), inv, 1e-6f * sm); dv = fmaf(E * (1.0f + vm), inv, 1e-6f * vm);
+    b.smin -= ds; b.smax += ds; b.vmin -= dv; b.vmax += dv;
 }
 
 // Does the box (camera frame: centre (Xc, Yc, Zc), half-edge vectors (Xx, Yx, Zx), (Xy, Yy, Zy), (Xz, 0, Zz)) reach
@@ -117,36 +135,105 @@ __device__ __forceinline__ bool cull_in_frustum(const CullPrim &q, float th, flo
     return true;
 }
 
-constexpr int kCullChunk = 320;        // primitives staged in shared memory per round
+// Precise pixel bounds of a box that straddles the clip plane X = near, or has a corner so close to it that the fast path's
+// uniform error term is too coarse: corners in front of the plane and the points where edges cross it are projected, each
+// with its own error term.  Returns (smin, smax, vmin, vmax); (-inf, inf, -inf, inf) = the whole image.  Out of line: it
+// runs for few primitives per view and must not cost the main path registers.
+__device__ __noinline__ float4 cull_bounds_precise(float Xc, float Yc, float Zc, float Xx, float Xy, float Xz, float Yx, float Yy,
+                                                   float Zx, float Zy, float Zz, float Xr, float E, float th, float tv, bool flat) {
+    const float near = kNearEps;
+    const float inf = __int_as_float(0x7f800000);
+    const float4 whole = make_float4(-inf, inf, -inf, inf);
+    if (Xc + Xr < near + E) return whole;                                 // thin sliver in front of the camera plane
+    PixBounds b = {3.0e38f, -3.0e38f, 3.0e38f, -3.0e38f, 3.0e38f};
+    const int nc = flat ? 4 : 8;                                          // flat: the corners c and c + 4 coincide
+    float cX[8], cY[8], cZ[8];
+#pragma unroll
+    for (int c = 0; c < 8; ++c) {
+        const float sx = (c & 1) ? 1.0f : -1.0f, sy = (c & 2) ? 1.0f : -1.0f, sz = (c & 4) ? 1.0f : -1.0f;
+        cX[c] = Xc + sx * Xx + sy * Xy + sz * Xz;
+        cY[c] = Yc + sx * Yx + sy * Yy;
+        cZ[c] = Zc + sx * Zx + sy * Zy + sz * Zz;
+    }
+    float qYmin = 3.0e38f, qYmax = -3.0e38f, qZmin = 3.0e38f, qZmax = -3.0e38f;   // cross-section at X = near
+#pragma unroll
+    for (int c = 0; c < 8; ++c) {
+        if (c >= nc) break;
+        if (cX[c] >= near) bound_point_err(b, cX[c], cY[c], cZ[c], E);
+#pragma unroll
+        for (int bit = 1; bit < 8; bit <<= 1) {
+            if ((c & bit) || bit >= nc) continue;
+            const int d = c | bit;
+            const float Xa = cX[c], Xb = cX[d];
+            if ((Xa < near) == (Xb < near)) continue;
+            const float t = (near - Xa) * rcp_fast(Xb - Xa);       // |Xb - Xa| > 0 here; error covered by E below
+            const float Yi = cY[c] + t * (cY[d] - cY[c]), Zi = cZ[c] + t * (cZ[d] - cZ[c]);
+            bound_point_err(b, near, Yi, Zi, E + 1e-6f * (fabsf(cY[d] - cY[c]) + fabsf(cZ[d] - cZ[c])));
+            qYmin = fminf(qYmin, Yi); qYmax = fmaxf(qYmax, Yi);
+            qZmin = fminf(qZmin, Zi); qZmax = fmaxf(qZmax, Zi);
+        }
+    }
+    // The part of the box with 0 < X < near is not covered by the bound above.  A point of it is inside
+    // the image only if |Y| < th X < th near and |Z| < tv near, i.e. only if the box reaches into the tip
+    // of the view pyramid; then give up and take the whole image.  Two conservative tests of that: the
+    // cross-section at X = near, and the camera-frame bounding intervals of the box, both against the tip
+    // widened to at least kNearGuard (the tip is large for extreme fields of view: tv near = 10 m at a
+    // 4096 x 4 image).  A box redone here only for precision lies wholly beyond the clip plane: nothing to guard.
+    if (Xc - Xr < near + E) {
+        const float gdY = fmaxf(kNearGuard, 1.01f * th * near) + E, gdZ = fmaxf(kNearGuard, 1.01f * tv * near) + E;
+        if (qYmin <= gdY && qYmax >= -gdY && qZmin <= gdZ && qZmax >= -gdZ) return whole;
+        if (fabsf(Yc) - (fabsf(Yx) + fabsf(Yy)) < gdY && fabsf(Zc) - (fabsf(Zx) + fabsf(Zy) + fabsf(Zz)) < gdZ &&
+            box_meets_tip(Xc, Yc, Zc, Xx, Xy, Xz, Yx, Yy, Zx, Zy, Zz, near, gdY, gdZ, E))   // rare
+            return whole;
+    }
+    return make_float4(b.smin, b.smax, b.vmin, b.vmax);
+}
+
+constexpr int kCullChunk = 320;        // primitives staged in shared memory per round (a multiple of 32)
 constexpr int kCullWarps = 8;          // views per CTA (one warp per view), all of the same world
 
+// Launch constants of the cull, formed once on the host (conservative geometry only, no contract arithmetic).
+struct CullArgs {
+    const gp_prim *prims; const float2 *pitch;
+    int world_begin, groups_per_world, H, W;
+    float th, tv;
+    float sth, stv;                    // |n| of the side planes (-th, +-1, 0) and (-tv, 0, +-1), times 1.0001
+    float msc;                         // 2 + th + tv
+    float inv_th, inv_tv, halfW, halfH;
+    float far_lim;                     // t_max (1 + 1e-6)
+    ViewHdr *hdr; EntryGeo *geo; EntryAux *aux; int cap;
+    unsigned long long *stats;
+};
+
 // Grid: one CTA per (world, group of kCullWarps views of that world).  The world's records (first 32 bytes of each:
-// centre, half extents, heading) are staged in shared memory once per CTA and shared by its views.
+// centre, half extents, heading) are staged in shared memory once per CTA and shared by its views, together with the
+// view-independent part of the phase-1 test (bounding-sphere radius with its error margin folded in).
 #ifndef GP_CULL_MIN_CTAS
 #define GP_CULL_MIN_CTAS 3
 #endif
 __global__ void __launch_bounds__(kCullWarps * 32, GP_CULL_MIN_CTAS)
-k_cull(SceneConst sc, const gp_prim *__restrict__ prims, const float2 *__restrict__ pitch,
-       int world_begin, int groups_per_world, int H, int W, float th, float tv,
-       ViewHdr *__restrict__ hdr, EntryGeo *__restrict__ geo, EntryAux *__restrict__ aux, int cap,
-       unsigned long long *__restrict__ stats) {
+k_cull(SceneConst sc, CullArgs ca) {
     __shared__ float4 s_p0[kCullChunk], s_p1[kCullChunk];
+    __shared__ float4 s_c[kCullChunk];                                   // phase 1: centre, R + E_k  (-inf: skip)
+    __shared__ float2 s_r[kCullChunk];                                   // phase 1: R sth + E_k msc, R stv + E_k msc
     __shared__ uint8_t s_sphere[kCullChunk];
-    __shared__ float s_R[kCullChunk];
     __shared__ uint16_t s_idx_all[kCullWarps][kCullChunk];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int wl = blockIdx.x / groups_per_world;                       // world within the rendered range
-    const int v = (blockIdx.x % groups_per_world) * kCullWarps + warp;  // view within the world
-    const bool active = v < sc.A * sc.C;                                // idle warps still join the barriers
-    const int a = v / sc.C, cam_id = v - a * sc.C;
-    const int view = wl * sc.A * sc.C + v;
+    const int wl = blockIdx.x / ca.groups_per_world;                    // world within the rendered range
+    const int v = (blockIdx.x - wl * ca.groups_per_world) * kCullWarps + warp;   // view within the world
+    const int vpw = sc.A * sc.C;
+    const bool active = v < vpw;                                        // idle warps still join the barriers
+    const int a = sc.C == 1 ? v : v / sc.C, cam_id = v - a * sc.C;
+    const int view = wl * vpw + v;
     uint16_t *s_idx = s_idx_all[warp];
     const unsigned lt_mask = (1u << lane) - 1u;
-    const int w = world_begin + wl;
-    const gp_prim *wp = prims + (size_t)w * sc.P;
+    const int w = ca.world_begin + wl;
+    const gp_prim *wp = ca.prims + (size_t)w * sc.P;
+    const float th = ca.th, tv = ca.tv;
+    const int H = ca.H, W = ca.W;
     CullCam cam = {};
     if (active) {
-        const float2 pc = __ldg(&pitch[(size_t)w * sc.A + a]);
+        const float2 pc = __ldg(&ca.pitch[(size_t)w * sc.A + a]);
         cam.cp = pc.x; cam.sp = pc.y;
         // C2 camera (contract operations)
         const float4 e0 = __ldg(reinterpret_cast<const float4 *>(&wp[a]));        // cx cy cz hx
@@ -160,27 +247,33 @@ k_cull(SceneConst sc, const gp_prim *__restrict__ prims, const float2 *__restric
         cam.ux = -c_mul(cam.sp, e_ck); cam.uy = -c_mul(cam.sp, e_sk);
     }
 
-    EntryGeo *vgeo = geo + (size_t)view * cap;
-    EntryAux *vaux = aux + (size_t)view * cap;
-    const float halfW = 0.5f * (float)W, halfH = 0.5f * (float)H;
-    const float inv_th = 1.0f / th, inv_tv = 1.0f / tv;
+    EntryGeo *vgeo = ca.geo + (size_t)view * ca.cap;
+    EntryAux *vaux = ca.aux + (size_t)view * ca.cap;
     int cnt = 0, rmin = 0x1fff;            // list length (warp-uniform), first row touched (per lane)
 
-    // bounding-sphere pre-test constants: |n| of the side planes (-th, +-1, 0) and (-tv, 0, +-1)
-    const float sth = sqrtf(fmaf(th, th, 1.0f)) * 1.0001f, stv = sqrtf(fmaf(tv, tv, 1.0f)) * 1.0001f;
-    const float far_lim = sc.t_max * (1.0f + 1e-6f);
-    const float msc = 2.0f + th + tv;
+    // Phase-1 error margin.  The camera-frame coordinates of a centre are formed from d = c - o in fp32; their absolute
+    // error is below 1e-5 (|d.x| + |d.y| + |d.z| + R) + 1e-6, and |d.m| <= |c.m| + |o.m|, so the margin splits into a
+    // per-primitive part E_k (staged with the record) and a per-view part E_cam.
+    const float Ecam = 1.0001e-5f * (fabsf(cam.ox) + fabsf(cam.oy) + fabsf(cam.oz));
+    const float EcamM = Ecam * ca.msc;
+    const float ninf = __int_as_float(0xff800000);
 
     for (int k0 = 0; k0 < sc.P; k0 += kCullChunk) {
         const int k1 = min(sc.P, k0 + kCullChunk);
         if (k0) __syncthreads();                                         // previous round fully consumed
-        for (int i = threadIdx.x; i < k1 - k0; i += blockDim.x) {
+        const int npad = (k1 - k0 + 31) & ~31;                           // phase 1 runs whole warps: pad with "skip"
+        for (int i = threadIdx.x; i < npad; i += blockDim.x) {
+            if (i >= k1 - k0) { s_c[i] = make_float4(0.0f, 0.0f, 0.0f, ninf); s_r[i] = make_float2(0.0f, 0.0f); continue; }
             const float4 *rec = reinterpret_cast<const float4 *>(&wp[k0 + i]);
             float4 p0 = __ldg(rec), p1 = __ldg(rec + 1);
             const bool sphere = __float_as_int(__ldg(rec + 2).z) == GP_SHAPE_SPHERE;     // cls inst shape pad
             if (sphere) { p1.x = p0.w; p1.y = p0.w; p1.z = 1.0f; p1.w = 0.0f; }          // bounding cube, heading 0
             s_p0[i] = p0; s_p1[i] = p1; s_sphere[i] = sphere;
-            s_R[i] = sqrtf(fmaf(p0.w, p0.w, fmaf(p1.x, p1.x, p1.y * p1.y))) * 1.0001f;      // bounding-sphere radius
+            const float R = sqrtf(fmaf(p0.w, p0.w, fmaf(p1.x, p1.x, p1.y * p1.y))) * 1.0001f;      // bounding-sphere radius
+            const float Ek = 1.0001f * fmaf(1e-5f, fabsf(p0.x) + fabsf(p0.y) + fabsf(p0.z) + R, 1e-6f);
+            const bool skip = sphere && !sc.spheres;
+            s_c[i] = make_float4(p0.x, p0.y, p0.z, skip ? ninf : R + Ek);
+            s_r[i] = make_float2(fmaf(R, ca.sth, Ek * ca.msc), fmaf(R, ca.stv, Ek * ca.msc));
         }
         __syncthreads();
         if (!active) continue;
@@ -188,23 +281,23 @@ k_cull(SceneConst sc, const gp_prim *__restrict__ prims, const float2 *__restric
         // frame (looser than the exact box test of phase 2 by construction: the support of the box
         // along any unit direction is <= R); survivors compacted (ballot) into s_idx
         int m = 0;
-        for (int kb = k0; kb < k1; kb += 32) {
-            const int k = kb + lane;
-            bool pass = false;
-            if (k < k1 && k != a && (sc.spheres || !s_sphere[k - k0])) {
-                const float4 p0 = s_p0[k - k0];                                           // cx cy cz hx
-                const float dx = p0.x - cam.ox, dy = p0.y - cam.oy, dz = p0.z - cam.oz;
-                const float R = s_R[k - k0];
-                const float X = fmaf(dx, cam.fx, fmaf(dy, cam.fy, dz * cam.sp));
-                const float Y = fmaf(dx, cam.rx, dy * cam.ry);
-                const float Z = fmaf(dx, cam.ux, fmaf(dy, cam.uy, dz * cam.cp));
-                const float E = fmaf(1e-5f, fabsf(dx) + fabsf(dy) + fabsf(dz) + R, 1e-6f);
-                const float mg = E * msc;
-                pass = X + R >= -E && X - R <= far_lim + E &&
-                       fabsf(Y) - th * X <= fmaf(R, sth, mg) && fabsf(Z) - tv * X <= fmaf(R, stv, mg);
-            }
+#pragma unroll 2
+        for (int ib = 0; ib < npad; ib += 32) {
+            const int i = ib + lane;
+            const float4 c = s_c[i];                                                      // cx cy cz R + E_k
+            const float2 r = s_r[i];
+            const float dx = c.x - cam.ox, dy = c.y - cam.oy, dz = c.z - cam.oz;
+            const float X = fmaf(dx, cam.fx, fmaf(dy, cam.fy, dz * cam.sp));
+            const float Y = fmaf(dx, cam.rx, dy * cam.ry);
+            const float Z = fmaf(dx, cam.ux, fmaf(dy, cam.uy, dz * cam.cp));
+            const float Ra = c.w + Ecam;                                                  // -inf for a skipped record
+            // the four slacks (behind the camera plane / beyond the far plane, side planes in Y and in Z), branch-free:
+            // pass iff none is negative
+            const float t1 = X + Ra, t2 = (ca.far_lim - X) + Ra;
+            const float t3 = fmaf(th, X, r.x + EcamM) - fabsf(Y), t4 = fmaf(tv, X, r.y + EcamM) - fabsf(Z);
+            const bool pass = fminf(fminf(t1, t2), fminf(t3, t4)) >= 0.0f && k0 + i != a;
             const unsigned mask = __ballot_sync(0xffffffffu, pass);
-            if (pass) s_idx[m + __popc(mask & lt_mask)] = (uint16_t)(k - k0);
+            if (pass) s_idx[m + __popc(mask & lt_mask)] = (uint16_t)i;
             m += __popc(mask);
         }
         __syncwarp();
@@ -228,73 +321,39 @@ k_cull(SceneConst sc, const gp_prim *__restrict__ prims, const float2 *__restric
         }
         const float E = q.E, Xc = q.Xc, Yc = q.Yc, Zc = q.Zc, Xr = q.Xr;
         const float Xx = q.Xx, Xy = q.Xy, Xz = q.Xz, Yx = q.Yx, Yy = q.Yy, Zx = q.Zx, Zy = q.Zy, Zz = q.Zz;
-        const float hz = q.hz;
-        const int nc = hz == 0.0f ? 4 : 8;        // flat: the corners c and c + 4 coincide
-        // corner projection with near-plane clipping
-        float cX[8], cY[8], cZ[8];
+        const bool flat = q.hz == 0.0f;           // flat: the corners c and c + 4 coincide (Xz = Zz = 0)
+        PixBounds b = {3.0e38f, -3.0e38f, 3.0e38f, -3.0e38f, 3.0e38f};
+        // Fast path: the box lies wholly in front of the clip plane (every corner has X >= near).  Corners are projected
+        // without error terms and the rectangle is widened once by the largest error any corner can have; if that costs
+        // more than a quarter of a pixel (a corner very close to the camera plane), the precise path redoes it.
+        bool precise = !(Xc - Xr >= kNearEps + E);
+        if (!precise) {
 #pragma unroll
-        for (int c = 0; c < 8; ++c) {
-            const float sx = (c & 1) ? 1.0f : -1.0f, sy = (c & 2) ? 1.0f : -1.0f, sz = (c & 4) ? 1.0f : -1.0f;
-            cX[c] = Xc + sx * Xx + sy * Xy + sz * Xz;
-            cY[c] = Yc + sx * Yx + sy * Yy;
-            cZ[c] = Zc + sx * Zx + sy * Zy + sz * Zz;
-        }
-        PixBounds b = {3.0e38f, -3.0e38f, 3.0e38f, -3.0e38f};
-        bool full = false;
-        const float near = kNearEps;
-        if (Xc - Xr >= near + E) {
-#pragma unroll
-            for (int c = 0; c < 4; ++c) bound_point(b, cX[c], cY[c], cZ[c], E);
-            if (nc == 8) {
-#pragma unroll
-                for (int c = 4; c < 8; ++c) bound_point(b, cX[c], cY[c], cZ[c], E);
+            for (int c = 0; c < 4; ++c) {
+                const float sx = (c & 1) ? 1.0f : -1.0f, sy = (c & 2) ? 1.0f : -1.0f;
+                const float Xb = Xc + sx * Xx + sy * Xy, Yb = Yc + sx * Yx + sy * Yy, Zb = Zc + sx * Zx + sy * Zy;
+                bound_point(b, Xb - Xz, Yb, Zb - Zz);
+                if (!flat) bound_point(b, Xb + Xz, Yb, Zb + Zz);
             }
-        } else if (Xc + Xr < near + E) {
-            full = true;                                                  // thin sliver in front of the camera plane
-        } else {
-            float qYmin = 3.0e38f, qYmax = -3.0e38f, qZmin = 3.0e38f, qZmax = -3.0e38f;   // cross-section at X = near
-#pragma unroll
-            for (int c = 0; c < 8; ++c) {
-                if (c >= nc) break;
-                if (cX[c] >= near) bound_point(b, cX[c], cY[c], cZ[c], E);
-#pragma unroll
-                for (int bit = 1; bit < 8; bit <<= 1) {
-                    if ((c & bit) || bit >= nc) continue;
-                    const int d = c | bit;
-                    const float Xa = cX[c], Xb = cX[d];
-                    if ((Xa < near) == (Xb < near)) continue;
-                    const float t = (near - Xa) * rcp_fast(Xb - Xa);       // |Xb - Xa| > 0 here; error covered by E below
-                    const float Yi = cY[c] + t * (cY[d] - cY[c]), Zi = cZ[c] + t * (cZ[d] - cZ[c]);
-                    bound_point(b, near, Yi, Zi, E + 1e-6f * (fabsf(cY[d] - cY[c]) + fabsf(cZ[d] - cZ[c])));
-                    qYmin = fminf(qYmin, Yi); qYmax = fmaxf(qYmax, Yi);
-                    qZmin = fminf(qZmin, Zi); qZmax = fmaxf(qZmax, Zi);
-                }
-            }
-            // The part of the box with 0 < X < near is not covered by the bound above.  A point of it is inside
-            // the image only if |Y| < th X < th near and |Z| < tv near, i.e. only if the box reaches into the tip
-            // of the view pyramid; then give up and take the whole image.  Two conservative tests of that: the
-            // cross-section at X = near, and the camera-frame bounding intervals of the box, both against the tip
-            // widened to at least kNearGuard (the tip is large for extreme fields of view: tv near = 10 m at a
-            // 4096 x 4 image).
-            const float gdY = fmaxf(kNearGuard, 1.01f * th * near) + E, gdZ = fmaxf(kNearGuard, 1.01f * tv * near) + E;
-            if (qYmin <= gdY && qYmax >= -gdY && qZmin <= gdZ && qZmax >= -gdZ) full = true;
-            if (!full && fabsf(Yc) - (fabsf(Yx) + fabsf(Yy)) < gdY && fabsf(Zc) - (fabsf(Zx) + fabsf(Zy) + fabsf(Zz)) < gdZ)
-                full = box_meets_tip(Xc, Yc, Zc, Xx, Xy, Xz, Yx, Yy, Zx, Zy, Zz, near, gdY, gdZ, E);   // rare
+            float ds, dv;
+            bound_widen(b, E, ds, dv);
+            precise = ds * (ca.inv_th * ca.halfW) > 0.25f || dv * (ca.inv_tv * ca.halfH) > 0.25f;
         }
-        int c0, c1, r0, r1;
-        if (full) { c0 = 0; c1 = W - 1; r0 = 0; r1 = H - 1; }
-        else {
-            // continuous pixel coordinate of s: (s/th + 1) W/2; pixel j is covered iff its centre j + 0.5 is inside
-            const float xl = fminf(fmaxf((b.smin * inv_th + 1.0f) * halfW - 0.52f, -1.0f), (float)W);
-            const float xh = fminf(fmaxf((b.smax * inv_th + 1.0f) * halfW - 0.48f, -1.0f), (float)W);
-            const float yl = fminf(fmaxf((1.0f - b.vmax * inv_tv) * halfH - 0.52f, -1.0f), (float)H);
-            const float yh = fminf(fmaxf((1.0f - b.vmin * inv_tv) * halfH - 0.48f, -1.0f), (float)H);
-            c0 = max((int)ceilf(xl), 0); c1 = min((int)floorf(xh), W - 1);
-            r0 = max((int)ceilf(yl), 0); r1 = min((int)floorf(yh), H - 1);
-            if (c0 > c1 || r0 > r1) keep = false;                         // touches no pixel centre
+        if (precise) {                                                    // few primitives per view; out of line (registers)
+            const float4 pb = cull_bounds_precise(Xc, Yc, Zc, Xx, Xy, Xz, Yx, Yy, Zx, Zy, Zz, Xr, E, th, tv, flat);
+            b.smin = pb.x; b.smax = pb.y; b.vmin = pb.z; b.vmax = pb.w;
         }
+        // continuous pixel coordinate of s: (s/th + 1) W/2; pixel j is covered iff its centre j + 0.5 is inside
+        // (bounds of +-inf, the whole image, clamp to it; an empty accumulation, 3e38 / -3e38, gives c0 > c1)
+        const float xl = fminf(fmaxf((b.smin * ca.inv_th + 1.0f) * ca.halfW - 0.52f, -1.0f), (float)W);
+        const float xh = fminf(fmaxf((b.smax * ca.inv_th + 1.0f) * ca.halfW - 0.48f, -1.0f), (float)W);
+        const float yl = fminf(fmaxf((1.0f - b.vmax * ca.inv_tv) * ca.halfH - 0.52f, -1.0f), (float)H);
+        const float yh = fminf(fmaxf((1.0f - b.vmin * ca.inv_tv) * ca.halfH - 0.48f, -1.0f), (float)H);
+        const int c0 = max((int)ceilf(xl), 0), c1 = min((int)floorf(xh), W - 1);
+        const int r0 = max((int)ceilf(yl), 0), r1 = min((int)floorf(yh), H - 1);
+        if (c0 > c1 || r0 > r1) keep = false;                             // touches no pixel centre
         if (keep) rmin = min(rmin, r0);
-        x.kf = ((uint32_t)k << 2) | (sphere ? kKindSphere : hz == 0.0f ? kKindFlat : kKindBox);
+        x.kf = ((uint32_t)k << 2) | (sphere ? kKindSphere : flat ? kKindFlat : kKindBox);
         x.rows = (uint32_t)r0 | ((uint32_t)r1 << 16);
         x.cols = (uint32_t)c0 | ((uint32_t)c1 << 16);
         x.pad = 0;
@@ -313,8 +372,8 @@ k_cull(SceneConst sc, const gp_prim *__restrict__ prims, const float2 *__restric
     rmin = __reduce_min_sync(0xffffffffu, rmin);
     if (lane == 0) {
         ViewHdr h; h.n = cnt | (rmin << 19); h.oz = cam.oz; h.cp = cam.cp; h.sp = cam.sp;
-        hdr[view] = h;
-        if (stats) atomicAdd(&stats[1], (unsigned long long)cnt);
+        ca.hdr[view] = h;
+        if (ca.stats) atomicAdd(&ca.stats[1], (unsigned long long)cnt);
     }
 }
 

@@ -45,4 +45,28 @@ k_probe_fma(int iters, float seed, float *out) {
     if (s != s) out[0] = s;
 }
 
+// Exhaustive check of c_rcp2 against __frcp_rn: every one of the 2^32 bit patterns, each paired with a few partners
+// (1, 0, 2^127, a subnormal, either sign) so that both outputs and both sides of the joint range check are exercised.
+// out[0] += mismatching patterns.
+__global__ void __launch_bounds__(256)
+k_probe_rcp(unsigned long long *out) {
+    unsigned long long bad = 0;
+    const uint32_t partners[4] = {0x3f800000u, 0x00000000u, 0x7f000000u, 0x00400000u};
+    for (unsigned long long b = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; b < (1ull << 32);
+         b += (unsigned long long)gridDim.x * blockDim.x) {
+        const float x = __uint_as_float((uint32_t)b);
+        const uint32_t want = __float_as_uint(__frcp_rn(x));
+        const float y = __uint_as_float(partners[b & 3] ^ (uint32_t)(b >> 7 << 31));
+        const uint32_t want_y = __float_as_uint(__frcp_rn(y));
+        float ix, iy;
+        c_rcp2(x, y, ix, iy);
+        bool ok = __float_as_uint(ix) == want && __float_as_uint(iy) == want_y;     // NaN in -> the same NaN bits out
+        c_rcp2(y, x, iy, ix);
+        ok = ok && __float_as_uint(ix) == want && __float_as_uint(iy) == want_y;
+        if (!ok) ++bad;
+    }
+    for (int o = 16; o; o >>= 1) bad += __shfl_xor_sync(0xffffffffu, bad, o);
+    if ((threadIdx.x & 31) == 0 && bad) atomicAdd(out, bad);
+}
+
 }  // namespace gp

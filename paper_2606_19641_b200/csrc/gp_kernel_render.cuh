@@ -27,6 +27,10 @@ struct RenderArgs {
     unsigned long long *stats;
     // raster variant (gp_kernel_raster.cuh): SR = rows per tile, log2W = -1 unless W is a power of two
     int ntiles;                     // tiles per view
+    // divisions by launch constants, as multiplications (host side: render_device)
+    int n_strips;                   // ceil(H / SR)
+    uint32_t magicSR;               // ceil(2^32 / SR): row / SR = umulhi(row, magicSR) for row < 8192
+    uint32_t magic_vpw; int shift_vpw;   // view / (A * C) = (view * magic_vpw) >> shift_vpw for view < 2^31
     float two_over_H, two_over_W;   // 2.0f / (float)H, 2.0f / (float)W: IEEE divisions done on the host (C2)
 };
 
@@ -165,7 +169,8 @@ __device__ __forceinline__ void slab_z(const float4 &g1, const float4 &rt, float
 template <bool ATOMIC>      // ATOMIC: other lanes of the warp may update the same key at the same time
 __device__ __forceinline__ void slab_select(const float4 &g0, float dlx, float dly, float loz, float hiz, float dz,
                                             float t_max, bool flat, uint32_t klow, unsigned long long *kp) {
-    const float ix = c_rcp(dlx), iy = c_rcp(dly);
+    float ix, iy;
+    c_rcp2(dlx, dly, ix, iy);                          // == c_rcp(dlx), c_rcp(dly)
     float ta, tb;
     ta = c_mul(g0.x, ix); tb = c_mul(g0.y, ix);
     const float lox = c_min(ta, tb), hix = c_max(ta, tb);
@@ -452,10 +457,10 @@ k_render(SceneConst sc, RenderArgs ra) {
     }
     __syncthreads();                       // tables + mbarrier init visible
 
-    const int w = ra.world_begin + view / (sc.A * sc.C);
+    const int w = ra.world_begin + (int)(((unsigned long long)(unsigned)view * ra.magic_vpw) >> ra.shift_vpw);   // view / (A C)
     const uint32_t *wtab = reinterpret_cast<const uint32_t *>(ra.meta + (size_t)w * sc.P);   // uint32[P][8]
     const size_t HW = (size_t)H * W;
-    const int n_strips = (H + SR - 1) / SR;
+    const int n_strips = ra.n_strips;
     // resolve pass: lane owns pixels 4*lane .. 4*lane+3 of every 128-pixel group of the strip
     const int lane_row = (lane * 4) / W, lane_col = (lane * 4) % W;
     const int step_row = 128 / W, step_col = 128 % W;
@@ -464,7 +469,7 @@ k_render(SceneConst sc, RenderArgs ra) {
     // Strip schedule: strips are handed out dynamically in ascending order (ascending addresses are
     // also what the HBM likes: a descending order measured 13% slower).  Strips wholly above the first
     // row any entry touches need no list and are rendered while the bulk copies are still in flight.
-    const int n_free = n > 0 ? min(n_strips, rmin / SR) : n_strips;
+    const int n_free = n > 0 ? min(n_strips, (int)__umulhi((unsigned)rmin, ra.magicSR)) : n_strips;    // rmin / SR
     const EntryGeo *g_geo = ra.geo + (size_t)view * ra.cap;
     const EntryAux *g_aux = ra.aux + (size_t)view * ra.cap;
     bool list_ready = false;
@@ -472,7 +477,8 @@ k_render(SceneConst sc, RenderArgs ra) {
     for (int strip_it = warp;; strip_it += n_warps) {
         int strip = strip_it;
         if (DYN) {                                                      // dynamic hand-out (balances long lists)
-            if (lane == 0) strip = atomicAdd(s_next, 1);
+            // (plain PTX: nvcc wraps atomicAdd in a warp-aggregation sequence of ~15 instructions, for one lane)
+            if (lane == 0) asm volatile("atom.shared.add.u32 %0, [%1], 1;" : "=r"(strip) : "r"(smem_u32(s_next)) : "memory");
             strip = __shfl_sync(0xffffffffu, strip, 0);
         }
         if (strip >= n_strips) break;

@@ -589,14 +589,23 @@ static int render_device(gp_ctx *c, int world_begin, int n_worlds, int H, int W,
         CK(cudaStreamWaitEvent(cull_stream, c->pipe_ev[n_chunks], 0));
     }
     const int gpw = (vpw + kCullWarps - 1) / kCullWarps;               // cull CTAs per world
+    CullArgs cargs{};
+    cargs.prims = c->d_prims; cargs.pitch = c->d_pitch; cargs.groups_per_world = gpw; cargs.H = H; cargs.W = W;
+    cargs.th = th; cargs.tv = tv;
+    cargs.sth = sqrtf(fmaf(th, th, 1.0f)) * 1.0001f; cargs.stv = sqrtf(fmaf(tv, tv, 1.0f)) * 1.0001f;
+    cargs.msc = 2.0f + th + tv;
+    cargs.inv_th = 1.0f / th; cargs.inv_tv = 1.0f / tv; cargs.halfW = 0.5f * (float)W; cargs.halfH = 0.5f * (float)H;
+    cargs.far_lim = sc.t_max * (1.0f + 1e-6f);
+    cargs.cap = c->scratch_cap; cargs.stats = stats;
     auto launch_cull = [&](int ci, cudaStream_t st) -> int {
         const int w0 = ci * wpc, nw = std::min(wpc, n_worlds - w0);
         const size_t v0 = (size_t)w0 * vpw;
+        CullArgs ca = cargs;
+        ca.world_begin = world_begin + w0;
+        ca.hdr = c->d_hdr + v0; ca.geo = c->d_geo + v0 * c->scratch_cap; ca.aux = c->d_aux + v0 * c->scratch_cap;
         {
             LaunchTimer lt(c, GP_KERNEL_CULL, st);
-            k_cull<<<(unsigned)((size_t)nw * gpw), kCullWarps * 32, 0, st>>>(
-                sc, c->d_prims, c->d_pitch, world_begin + w0, gpw, H, W, th, tv, c->d_hdr + v0,
-                c->d_geo + v0 * c->scratch_cap, c->d_aux + v0 * c->scratch_cap, c->scratch_cap, stats);
+            k_cull<<<(unsigned)((size_t)nw * gpw), kCullWarps * 32, 0, st>>>(sc, ca);
         }
         c->launches += 1;
         CK(cudaGetLastError());
@@ -626,6 +635,8 @@ static int render_device(gp_ctx *c, int world_begin, int n_worlds, int H, int W,
         ctas_per_view = (unsigned)rp.ntiles; block = (unsigned)rp.nwarps * 32; smem = rp.smem;
     } else {
         ra.scap = pl.scap; ra.SR = pl.SR; ra.log2LC = pl.log2LC; ra.log2W = pl.log2W; ra.ngr = pl.ngr; ra.magicW = pl.magicW;
+        ra.n_strips = (H + pl.SR - 1) / pl.SR;
+        ra.magicSR = (uint32_t)((0x100000000ull + (unsigned)pl.SR - 1) / (unsigned)pl.SR);
 #define GP_FNS(ST, SP, GA) {k_render<ST, 0, SP, GA>, k_render<ST, 1, SP, GA>, k_render<ST, 2, SP, GA>, k_render<ST, 4, SP, GA>}
         static const RenderFn fns[2][2][2][4] = {      // [gather][spheres][stats][ng index]
             {{GP_FNS(false, false, false), GP_FNS(true, false, false)}, {GP_FNS(false, true, false), GP_FNS(true, true, false)}},
@@ -641,6 +652,12 @@ static int render_device(gp_ctx *c, int world_begin, int n_worlds, int H, int W,
         }
         fn = fns[pl.gather][spheres ? 1 : 0][stats ? 1 : 0][pl.ng == 4 ? 3 : pl.ng];
         block = (unsigned)pl.nwarps * 32; smem = pl.smem;
+    }
+    {   // view / vpw for view < 2^31: (view * ceil(2^(31 + L) / vpw)) >> (31 + L), L = ceil(log2 vpw) (round-up method)
+        int L = 0;
+        while ((1ll << L) < vpw) ++L;
+        ra.shift_vpw = 31 + L;
+        ra.magic_vpw = (uint32_t)(((1ull << (31 + L)) + (unsigned)vpw - 1) / (unsigned)vpw);
     }
     const size_t HW = (size_t)H * W;
     rc = launch_cull(0, stream);                                       // chunk 0: nothing to overlap with yet
@@ -764,6 +781,10 @@ extern "C" int gp_probe(gp_ctx *c, int kind, size_t n_pixels, int iters, uint8_t
             const int reps = 4096;
             k_probe_fma<<<148 * 8, 256, 0, stream>>>(reps, 1.0f + (float)it, reinterpret_cast<float *>(c->d_stats));
             units = 2.0 * 148.0 * 8 * 256 * (double)reps * 16 * 8 / 1e12;       // TFLOP
+        } else if (kind == GP_PROBE_RCP) {
+            if (it == 0) CK(cudaMemsetAsync(c->d_stats, 0, sizeof(unsigned long long), stream));   // count over all launches
+            k_probe_rcp<<<148 * 8, 256, 0, stream>>>(c->d_stats);
+            units = 0.0;
         } else { rc = GP_ERR_ARG; break; }
         c->launches += 1;
         cudaEventRecord(e1, stream);
@@ -774,6 +795,14 @@ extern "C" int gp_probe(gp_ctx *c, int kind, size_t n_pixels, int iters, uint8_t
     }
     cudaEventDestroy(e0); cudaEventDestroy(e1);
     if (rc != GP_OK) return rc;
+    if (kind == GP_PROBE_RCP) {                                                 // result = mismatching bit patterns
+        unsigned long long bad = 0;
+        CK(cudaMemcpy(&bad, c->d_stats, sizeof bad, cudaMemcpyDeviceToHost));
+        CK(cudaMemset(c->d_stats, 0, sizeof bad));
+        *best = (double)bad;
+        if (median) *median = (double)bad;
+        return GP_OK;
+    }
     std::sort(rate.begin(), rate.end());
     *best = rate.back();
     if (median) *median = rate[rate.size() / 2];

@@ -20,7 +20,7 @@ GP_OPT_VARIANT, GP_OPT_TILE_PX, GP_OPT_PIPELINE = 8, 9, 10
 GP_VARIANT_RAY, GP_VARIANT_RASTER = 0, 1
 GP_KERNEL_UPDATE, GP_KERNEL_CULL, GP_KERNEL_RENDER, GP_KERNEL_BRUTE, GP_KERNEL_DYNAMICS, GP_KERNEL_OBSERVE = 0, 1, 2, 3, 4, 5
 GP_PATH_FAST, GP_PATH_BRUTE = 0, 1
-GP_PROBE_STORE, GP_PROBE_FMA = 0, 1
+GP_PROBE_STORE, GP_PROBE_FMA, GP_PROBE_RCP = 0, 1, 2
 
 EXPORTS = ("gp_create", "gp_destroy", "gp_set_option", "gp_scene_upload", "gp_agents_update",
            "gp_cameras_set", "gp_render_batch", "gp_render_batch_host", "gp_stats", "gp_kernel_time",
