@@ -209,7 +209,7 @@ struct CullArgs {
 // centre, half extents, heading) are staged in shared memory once per CTA and shared by its views, together with the
 // view-independent part of the phase-1 test (bounding-sphere radius with its error margin folded in).
 #ifndef GP_CULL_MIN_CTAS
-#define GP_CULL_MIN_CTAS 3
+#define GP_CULL_MIN_CTAS 4
 #endif
 __global__ void __launch_bounds__(kCullWarps * 32, GP_CULL_MIN_CTAS)
 k_cull(SceneConst sc, CullArgs ca) {
