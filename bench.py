@@ -318,8 +318,13 @@ def run_b200(args):
         n_probe = (min(cfg.views, chunk * vpw) * cfg.H * cfg.W) // 128 * 128
         st_best, st_med = r.probe(gp.GP_PROBE_STORE, n_probe, 10, outs)
         fma_best, fma_med = r.probe(gp.GP_PROBE_FMA, 0, 10)
+        sv_best = sv_med = None
+        if (cfg.H * cfg.W) % 128 == 0:          # the same stream, one CTA per view as k_render maps it
+            n_view = min(cfg.views, chunk * vpw) * cfg.H * cfg.W
+            sv_best, sv_med = r.probe(gp.GP_PROBE_STORE_VIEW, n_view, 10, outs)
         probes = {"store_gbs_best": st_best, "store_gbs_median": st_med, "store_bytes": n_probe * 12,
                   "fma_tflops_best": fma_best, "fma_tflops_median": fma_med,
+                  "store_view_gbs_best": sv_best, "store_view_gbs_median": sv_med,
                   "how": "gp_probe: 10 launches after 1 warm-up each, CUDA events; store = 12 B/px plane pattern of k_render over "
                          "the bench's own output planes; fma = 8 FFMA chains/thread, 148x8 CTAs x 256 threads"}
     except Exception as ex:  # noqa: BLE001
@@ -447,6 +452,7 @@ def run_b200(args):
     fp32_nominal = 148 * 128 * 2 * sm_mhz * 1e6
     fp32_peak = (probes or {}).get("fma_tflops_best", 0) * 1e12 or fp32_nominal
     wr_peak = (probes or {}).get("store_gbs_best")
+    wv_peak = (probes or {}).get("store_view_gbs_best")
     t_fp32_ms = stats["executed_tests"] * FP32_OPS_PER_TEST / fp32_peak * 1e3
     t_hbm_ms = alg_bytes / (peak * 1e9) * 1e3
     step_ms = ms / args.steps
@@ -465,6 +471,9 @@ def run_b200(args):
                      "frac": achieved / peak, "traffic": traffic, "traffic_source": traffic_source, "peak_source": peak_src,
                      "peak_write_only": wr_peak, "frac_write_only": (achieved / wr_peak) if wr_peak else None,
                      "peak_write_only_source": "gp_probe(GP_PROBE_STORE) in this run: write-only kernel with k_render's store pattern",
+                     "peak_view_pattern": wv_peak, "frac_view_pattern": (achieved / wv_peak) if wv_peak else None,
+                     "peak_view_pattern_source": "gp_probe(GP_PROBE_STORE_VIEW) in this run: the same write-only stream with "
+                                                 "k_render's CTA -> address mapping (one CTA per view)",
                      "algorithmic_bytes_per_launch": alg_bytes_launch, "avg_launch_ms": r_avg_ms,
                      "launches_per_step": render_launches_per_step, "share_of_step": r_ms / steps_sampled / step_ms,
                      "note": "the culls of later world chunks run concurrently with these launches on a second stream"},

@@ -184,10 +184,18 @@ int gp_camera_rig_set(gp_ctx *ctx, int n_cams, const gp_camera *h_rig);
  * 1 <= H, W <= 4096.  The fast path needs W >= 4 and (H * W) % 4 == 0 (e.g. 210 x 126, 434 x 252) and one
  * warp's strip of the image in shared memory (fails only for widths near 4096 that are not a multiple of 4);
  * other sizes take the brute-force path, with identical results.
- * May grow library-owned scratch on first use of a larger (n_worlds, H, W): warm up before timing. */
+ * May grow library-owned scratch on first use of a larger (n_worlds, H, W) — a device synchronisation and a
+ * cudaMalloc —: call gp_reserve first (or warm up) where that must not happen inside the step. */
 int gp_render_batch(gp_ctx *ctx, int world_begin, int n_worlds, int agents, int H, int W,
                     float fov_rad, uint8_t *d_class, int32_t *d_instance, float *d_depth,
                     uint8_t *d_rgb, void *stream);
+
+/* Sizes the library-owned per-view scratch (list headers and lists of the cull) for render calls of up to n_worlds worlds
+ * with the current rig, and opts the render kernels into the shared memory an H x W image needs.  After it,
+ * gp_render_batch with n_worlds' <= n_worlds at that image size allocates nothing and does not synchronise the device.
+ * Synchronises the device if it has to grow the scratch.  Call it again after gp_camera_rig_set changed the number of
+ * cameras.  GP_ERR_STATE before gp_scene_upload, GP_ERR_RANGE if n_worlds exceeds the scene, GP_ERR_NOMEM. */
+int gp_reserve(gp_ctx *ctx, int n_worlds, int H, int W);
 
 /* End-to-end variant with HOST buffers: copies h_pose (HOST [Wn][A][4], may be NULL = keep poses) to the
  * device, updates the agents, renders worlds [world_begin, world_begin+n_worlds) in chunks through
@@ -255,11 +263,15 @@ int gp_observe_vec(gp_ctx *ctx, const float *d_state, int K, int M, float radius
  *     pixels in all; their content is overwritten).  Result: GB/s.
  *   GP_PROBE_FMA: 8 independent FFMA chains per thread on 148 x 8 CTAs x 256 threads, no memory traffic; the plane
  *     pointers and n_pixels are ignored.  Result: TFLOP/s (2 flop per FFMA) at the clock the GPU runs this at.
+ *   GP_PROBE_STORE_VIEW: the same store stream with the render pass's CTA -> address mapping: one CTA per view of the
+ *     image size of the last gp_render_batch (H * W a multiple of 128; GP_ERR_STATE before any render), n_pixels a
+ *     multiple of H * W, colour planes laid out [view][3][H*W].  Result: GB/s.  The gap to GP_PROBE_STORE is what one
+ *     CTA per view costs in DRAM locality; k_render is measured against both.
  *   GP_PROBE_RCP: self-check of the render pass's paired reciprocal (C0: 1.0f / x correctly rounded) against
  *     __frcp_rn on all 2^32 bit patterns; the plane pointers and n_pixels are ignored.  Result: the number of bit
  *     patterns whose result differed, summed over the launches (0 = identical).
  * Runs `iters` timed launches after one warm-up; *best = highest rate, *median (may be NULL) = the median. */
-enum { GP_PROBE_STORE = 0, GP_PROBE_FMA = 1, GP_PROBE_RCP = 2 };
+enum { GP_PROBE_STORE = 0, GP_PROBE_FMA = 1, GP_PROBE_RCP = 2, GP_PROBE_STORE_VIEW = 3 };
 int gp_probe(gp_ctx *ctx, int kind, size_t n_pixels, int iters, uint8_t *d_class, int32_t *d_instance, float *d_depth,
              uint8_t *d_rgb, void *stream, double *best, double *median);
 

@@ -26,6 +26,27 @@ k_probe_store(size_t n_groups, uint8_t *o_cls, int32_t *o_inst, float *o_depth, 
     }
 }
 
+// The same 12 B / pixel store stream, but with the render pass's CTA -> address mapping: one CTA of 4 warps per "view" of
+// view_groups 128-pixel groups (the colour planes laid out [view][3][HW] as gp_render_batch writes them), warps taking
+// strips of 4 groups in ascending order.  The CTAs resident at one time (148 x 8) then write 1184 separate windows of every
+// plane instead of one compact one, which is what bounds k_render's own store stream.
+__global__ void __launch_bounds__(128, 8)
+k_probe_store_view(int view_groups, uint8_t *o_cls, int32_t *o_inst, float *o_depth, uint8_t *o_rgb, uint32_t val) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const size_t HW = (size_t)view_groups * 128, v0 = (size_t)blockIdx.x * HW;
+    for (int q0 = warp * 4; q0 < view_groups; q0 += 16)
+        for (int q = q0; q < min(q0 + 4, view_groups); ++q) {
+            const size_t oi = (size_t)q * 128 + lane * 4, o = v0 + oi;
+            *reinterpret_cast<uint32_t *>(o_cls + o) = val;
+            *reinterpret_cast<int4 *>(o_inst + o) = make_int4(-1, -1, -1, -1);
+            *reinterpret_cast<float4 *>(o_depth + o) = make_float4(1.0f, 1.0f, 1.0f, 1.0f);
+            uint8_t *pr = o_rgb + 3 * v0 + oi;
+            *reinterpret_cast<uint32_t *>(pr) = val;
+            *reinterpret_cast<uint32_t *>(pr + HW) = val;
+            *reinterpret_cast<uint32_t *>(pr + 2 * HW) = val;
+        }
+}
+
 // FP32 FMA throughput: 8 independent dependent-chains of FFMA per thread, no memory traffic; out is written only if a
 // result is NaN (never), which keeps the chains alive.
 __global__ void __launch_bounds__(256)

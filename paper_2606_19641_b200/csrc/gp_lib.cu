@@ -44,6 +44,7 @@ struct gp_ctx {
     uint64_t launches = 0;
     unsigned timing_seq[8] = {0, 0, 0, 0, 0, 0, 0, 0};
     size_t obs_smem_set = 0;
+    int last_H = 0, last_W = 0;                                  // image size of the last gp_render_batch (GP_PROBE_STORE_VIEW)
     size_t render_smem_set = 0, raster_smem_set = 0;
     // gp_render_batch_host staging
     float *d_pose = nullptr;
@@ -521,6 +522,34 @@ static bool plan_raster(const gp_ctx *c, const SceneConst &sc, int H, int W, Ras
     return pl.smem <= 227 * 1024;
 }
 
+// The render kernels by template arguments, and their dynamic shared-memory opt-in (raised, never lowered).
+typedef void (*RenderFn)(SceneConst, RenderArgs);
+#define GP_FNS(ST, SP, GA) {k_render<ST, 0, SP, GA>, k_render<ST, 1, SP, GA>, k_render<ST, 2, SP, GA>, k_render<ST, 4, SP, GA>}
+static const RenderFn kRenderFns[2][2][2][4] = {      // [gather][spheres][stats][ng index]
+    {{GP_FNS(false, false, false), GP_FNS(true, false, false)}, {GP_FNS(false, true, false), GP_FNS(true, true, false)}},
+    {{GP_FNS(false, false, true), GP_FNS(true, false, true)}, {GP_FNS(false, true, true), GP_FNS(true, true, true)}}};
+#undef GP_FNS
+static const RenderFn kRasterFns[2][2] = {{k_raster<false, false>, k_raster<true, false>},
+                                          {k_raster<false, true>, k_raster<true, true>}};     // [spheres][stats]
+static int set_render_smem(gp_ctx *c, size_t smem) {
+    if (smem <= c->render_smem_set) return GP_OK;
+    for (int ga = 0; ga < 2; ++ga)
+        for (int f = 0; f < 2; ++f)
+            for (int st = 0; st < 2; ++st)
+                for (int g = 0; g < 4; ++g)
+                    CK(cudaFuncSetAttribute(kRenderFns[ga][f][st][g], cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    c->render_smem_set = smem;
+    return GP_OK;
+}
+static int set_raster_smem(gp_ctx *c, size_t smem) {
+    if (smem <= c->raster_smem_set) return GP_OK;
+    for (int f = 0; f < 2; ++f)
+        for (int st = 0; st < 2; ++st)
+            CK(cudaFuncSetAttribute(kRasterFns[f][st], cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    c->raster_smem_set = smem;
+    return GP_OK;
+}
+
 // Enqueue cull + render (or the brute-force kernel) for a world range into DEVICE planes.
 static int render_device(gp_ctx *c, int world_begin, int n_worlds, int H, int W, float fov_rad,
                          uint8_t *d_class, int32_t *d_instance, float *d_depth, uint8_t *d_rgb,
@@ -531,6 +560,7 @@ static int render_device(gp_ctx *c, int world_begin, int n_worlds, int H, int W,
     const bool spheres = c->opt_spheres >= 0 ? c->opt_spheres != 0 : (c->has_spheres || c->statics_touched);
     SceneConst sc = c->sc;
     sc.spheres = spheres ? 1 : 0;
+    c->last_H = H; c->last_W = W;
     const float th = (float)tan(0.5 * (double)fov_rad);          // C2, host side
     const float tv = th * ((float)H / (float)W);
     const size_t views = (size_t)n_worlds * sc.A * sc.C;
@@ -616,41 +646,23 @@ static int render_device(gp_ctx *c, int world_begin, int n_worlds, int H, int W,
     ra.meta = c->d_meta;
     ra.two_over_H = 2.0f / (float)H; ra.two_over_W = 2.0f / (float)W;
     ra.cap = c->scratch_cap; ra.H = H; ra.W = W; ra.th = th; ra.tv = tv; ra.stats = stats;
-    typedef void (*RenderFn)(SceneConst, RenderArgs);
     RenderFn fn = nullptr;
     unsigned ctas_per_view = 1, block = 0;
     size_t smem = 0;
     if (variant == GP_VARIANT_RASTER) {
         ra.scap = rp.scap; ra.SR = rp.TR; ra.log2LC = rp.log2LC; ra.log2W = rp.wshift; ra.magicW = rp.magicW; ra.ntiles = rp.ntiles;
-        static const RenderFn rfns[2][2] = {{k_raster<false, false>, k_raster<true, false>},
-                                            {k_raster<false, true>, k_raster<true, true>}};     // [spheres][stats]
-        if (rp.smem > c->raster_smem_set) {
-            for (int f = 0; f < 2; ++f)
-                for (int st = 0; st < 2; ++st)
-                    CK(cudaFuncSetAttribute(rfns[f][st], cudaFuncAttributeMaxDynamicSharedMemorySize, (int)rp.smem));
-            c->raster_smem_set = rp.smem;
-        }
+        rc = set_raster_smem(c, rp.smem);
+        if (rc != GP_OK) return rc;
         if (views * (size_t)rp.ntiles > 0x7fffffffull) return GP_ERR_ARG;
-        fn = rfns[spheres ? 1 : 0][stats ? 1 : 0];
+        fn = kRasterFns[spheres ? 1 : 0][stats ? 1 : 0];
         ctas_per_view = (unsigned)rp.ntiles; block = (unsigned)rp.nwarps * 32; smem = rp.smem;
     } else {
         ra.scap = pl.scap; ra.SR = pl.SR; ra.log2LC = pl.log2LC; ra.log2W = pl.log2W; ra.ngr = pl.ngr; ra.magicW = pl.magicW;
         ra.n_strips = (H + pl.SR - 1) / pl.SR;
         ra.magicSR = (uint32_t)((0x100000000ull + (unsigned)pl.SR - 1) / (unsigned)pl.SR);
-#define GP_FNS(ST, SP, GA) {k_render<ST, 0, SP, GA>, k_render<ST, 1, SP, GA>, k_render<ST, 2, SP, GA>, k_render<ST, 4, SP, GA>}
-        static const RenderFn fns[2][2][2][4] = {      // [gather][spheres][stats][ng index]
-            {{GP_FNS(false, false, false), GP_FNS(true, false, false)}, {GP_FNS(false, true, false), GP_FNS(true, true, false)}},
-            {{GP_FNS(false, false, true), GP_FNS(true, false, true)}, {GP_FNS(false, true, true), GP_FNS(true, true, true)}}};
-#undef GP_FNS
-        if (pl.smem > c->render_smem_set) {
-            for (int ga = 0; ga < 2; ++ga)
-                for (int f = 0; f < 2; ++f)
-                    for (int st = 0; st < 2; ++st)
-                        for (int g = 0; g < 4; ++g)
-                            CK(cudaFuncSetAttribute(fns[ga][f][st][g], cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem));
-            c->render_smem_set = pl.smem;
-        }
-        fn = fns[pl.gather][spheres ? 1 : 0][stats ? 1 : 0][pl.ng == 4 ? 3 : pl.ng];
+        rc = set_render_smem(c, pl.smem);
+        if (rc != GP_OK) return rc;
+        fn = kRenderFns[pl.gather][spheres ? 1 : 0][stats ? 1 : 0][pl.ng == 4 ? 3 : pl.ng];
         block = (unsigned)pl.nwarps * 32; smem = pl.smem;
     }
     {   // view / vpw for view < 2^31: (view * ceil(2^(31 + L) / vpw)) >> (31 + L), L = ceil(log2 vpw) (round-up method)
@@ -681,6 +693,24 @@ static int render_device(gp_ctx *c, int world_begin, int n_worlds, int H, int W,
         }
         c->launches += 1;
         CK(cudaGetLastError());
+    }
+    return GP_OK;
+}
+
+extern "C" int gp_reserve(gp_ctx *c, int n_worlds, int H, int W) {
+    if (!c) return GP_ERR_ARG;
+    if (!c->have_scene) return GP_ERR_STATE;
+    if (H < 1 || W < 1 || H > 4096 || W > 4096 || n_worlds < 1) return GP_ERR_ARG;
+    if (n_worlds > c->sc.Wn) return GP_ERR_RANGE;
+    GP_ON_DEVICE(c);
+    const size_t views = (size_t)n_worlds * c->sc.A * c->sc.C;
+    if (views > 0x7fffffffull) return GP_ERR_ARG;
+    int rc = ensure_scratch(c, views);
+    if (rc != GP_OK) return rc;
+    if (W >= 4 && !(((long long)H * W) & 3)) {
+        RenderPlan pl{}; RasterPlan rp{};
+        if (plan_render(c, c->sc, H, W, pl) && (rc = set_render_smem(c, pl.smem)) != GP_OK) return rc;
+        if (plan_raster(c, c->sc, H, W, rp) && (rc = set_raster_smem(c, rp.smem)) != GP_OK) return rc;
     }
     return GP_OK;
 }
@@ -776,6 +806,15 @@ extern "C" int gp_probe(gp_ctx *c, int kind, size_t n_pixels, int iters, uint8_t
             const size_t groups = n_pixels / 128;
             k_probe_store<<<(unsigned)((groups + 15) / 16), 128, 0, stream>>>(groups, d_class, d_instance, d_depth, d_rgb,
                                                                                 n_pixels, 0x01010101u * (uint32_t)(it & 3));
+            units = (double)n_pixels * 12.0 / 1e9;                              // GB
+        } else if (kind == GP_PROBE_STORE_VIEW) {
+            const size_t HW = (size_t)c->last_H * c->last_W;
+            if (HW == 0) { rc = GP_ERR_STATE; break; }
+            if (!d_class || !d_instance || !d_depth || !d_rgb || (HW & 127) || n_pixels < HW || n_pixels % HW ||
+                n_pixels / HW > 0x7fffffffull) { rc = GP_ERR_ARG; break; }
+            if (!aligned16(d_class) || !aligned16(d_instance) || !aligned16(d_depth) || !aligned16(d_rgb)) { rc = GP_ERR_ALIGN; break; }
+            k_probe_store_view<<<(unsigned)(n_pixels / HW), 128, 0, stream>>>((int)(HW / 128), d_class, d_instance, d_depth, d_rgb,
+                                                                              0x01010101u * (uint32_t)(it & 3));
             units = (double)n_pixels * 12.0 / 1e9;                              // GB
         } else if (kind == GP_PROBE_FMA) {
             const int reps = 4096;

@@ -20,12 +20,12 @@ GP_OPT_VARIANT, GP_OPT_TILE_PX, GP_OPT_PIPELINE = 8, 9, 10
 GP_VARIANT_RAY, GP_VARIANT_RASTER = 0, 1
 GP_KERNEL_UPDATE, GP_KERNEL_CULL, GP_KERNEL_RENDER, GP_KERNEL_BRUTE, GP_KERNEL_DYNAMICS, GP_KERNEL_OBSERVE = 0, 1, 2, 3, 4, 5
 GP_PATH_FAST, GP_PATH_BRUTE = 0, 1
-GP_PROBE_STORE, GP_PROBE_FMA, GP_PROBE_RCP = 0, 1, 2
+GP_PROBE_STORE, GP_PROBE_FMA, GP_PROBE_RCP, GP_PROBE_STORE_VIEW = 0, 1, 2, 3
 
 EXPORTS = ("gp_create", "gp_destroy", "gp_set_option", "gp_scene_upload", "gp_agents_update",
            "gp_cameras_set", "gp_render_batch", "gp_render_batch_host", "gp_stats", "gp_kernel_time",
            "gp_launch_count", "gp_camera_rig_set", "gp_statics_from_polylines", "gp_statics_update",
-           "gp_dynamics_step", "gp_observe_vec", "gp_probe", "gp_error_string")
+           "gp_dynamics_step", "gp_observe_vec", "gp_probe", "gp_reserve", "gp_error_string")
 
 
 class SceneDesc(ctypes.Structure):
@@ -86,6 +86,7 @@ def lib():
         L.gp_observe_vec.argtypes = [vp, vp, ci, ci, cf, vp, vp, vp, vp, vp]
         L.gp_probe.argtypes = [vp, ci, ctypes.c_size_t, ci, vp, vp, vp, vp, vp, ctypes.POINTER(ctypes.c_double),
                                ctypes.POINTER(ctypes.c_double)]
+        L.gp_reserve.argtypes = [vp, ci, ci, ci]
         L.gp_error_string.argtypes = [ci]
         L.gp_error_string.restype = ctypes.c_char_p
         for name in EXPORTS[:-1]:
@@ -236,6 +237,10 @@ class Renderer:
         a = ctypes.c_uint64()
         _check(lib().gp_launch_count(self._h, ctypes.byref(a)))
         return a.value
+
+    def reserve(self, n_worlds, H, W):
+        """Size the per-view scratch so that render_batch(..., n_worlds' <= n_worlds, H, W, ...) allocates nothing."""
+        _check(lib().gp_reserve(self._h, int(n_worlds), int(H), int(W)))
 
     def alloc_outputs(self, n_views, H, W, rgb=True):
         import torch
