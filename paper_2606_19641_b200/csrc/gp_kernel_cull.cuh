@@ -17,6 +17,9 @@
 
 namespace gp {
 
+#ifndef GP_PDL
+#define GP_PDL 1
+#endif
 constexpr float kNearEps = 0.01f;      // clip plane for the projection bound, metres of planar depth
 constexpr float kNearGuard = 0.05f;    // cross-section this close to the optical centre => whole image
 
@@ -218,6 +221,11 @@ k_cull(SceneConst sc, CullArgs ca) {
     __shared__ float2 s_r[kCullChunk];                                   // phase 1: R sth + E_k msc, R stv + E_k msc
     __shared__ uint8_t s_sphere[kCullChunk];
     __shared__ uint16_t s_idx_all[kCullWarps][kCullChunk];
+#if GP_PDL
+    // let the render pass (launched with programmatic stream serialisation) start its view-independent prologue as this
+    // grid's CTAs drain; it waits (griddepcontrol.wait) for this grid to complete before it reads the lists
+    asm volatile("griddepcontrol.launch_dependents;");
+#endif
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int wl = blockIdx.x / ca.groups_per_world;                    // world within the rendered range
     const int v = (blockIdx.x - wl * ca.groups_per_world) * kCullWarps + warp;   // view within the world

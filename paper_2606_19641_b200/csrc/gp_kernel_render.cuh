@@ -53,6 +53,10 @@ __device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t by
                  ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
 }
 
+#ifndef GP_PDL
+#define GP_PDL 1
+#endif
+
 constexpr unsigned long long kKeyEmpty = 0xFFFFFFFFFFFFFFFFull;
 
 // 1/x to ~1 ulp in one MUFU instruction, for the conservative (non-contract) column-interval bound of flat
@@ -419,9 +423,7 @@ k_render(SceneConst sc, RenderArgs ra) {
     unsigned long long *s_keys = reinterpret_cast<unsigned long long *>(s_olist + (GATHER ? (blockDim.x >> 5) * kOverlapCap : 0));
     unsigned long long *keys = s_keys + (size_t)warp * SR * W;
 
-    const float4 vh4 = __ldg(reinterpret_cast<const float4 *>(&ra.hdr[view]));
-    ViewHdr vh; vh.n = __float_as_int(vh4.x); vh.oz = vh4.y; vh.cp = vh4.z; vh.sp = vh4.w;
-    const int n = vh.n & 0x7ffff, rmin = (int)((uint32_t)vh.n >> 19);
+    // ---- view-independent part of the prologue (runs ahead of the cull's last CTAs under programmatic dependent launch) ----
     int *s_next = reinterpret_cast<int *>(smem + 8);               // dynamic strip counter
     if (threadIdx.x == 32 % blockDim.x) {
         const uint32_t g = shade_rgb(sc.pal[1], shade_scale(c_max(sc.Lz, 0.0f), sc.ambient)), k = sc.pal[0];
@@ -433,17 +435,26 @@ k_render(SceneConst sc, RenderArgs ra) {
         *s_next = 0;
         mbar_init(bar, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        if (n > 0) {
-            const uint32_t ns = (uint32_t)min(n, ra.scap);   // entries beyond scap are read from global memory
-            mbar_expect_tx(bar, ns * 64u);
-            bulk_g2s(s_geo, ra.geo + (size_t)view * ra.cap, ns * 48u, bar);
-            bulk_g2s(s_aux, ra.aux + (size_t)view * ra.cap, ns * 16u, bar);
-        }
     }
-    // tables (contract C2-C4), overlapped with the bulk copies
-    // (2 / W and 2 / H are IEEE divisions done once on the host: the same fp32 numbers pix_s / pix_v form)
+    // column table (contract C2; 2 / W and 2 / H are IEEE divisions done once on the host: the same fp32 numbers pix_s /
+    // pix_v form)
     for (int j = threadIdx.x; j < W; j += blockDim.x)
         s_col[j] = c_mul(c_sub(c_mul(c_add((float)j, 0.5f), ra.two_over_W), 1.0f), ra.th);
+#if GP_PDL
+    // Programmatic dependent launch: wait for the cull's grid before the first read of what it wrote (returns at once when
+    // the kernel was launched normally).
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+#endif
+    const float4 vh4 = __ldg(reinterpret_cast<const float4 *>(&ra.hdr[view]));
+    ViewHdr vh; vh.n = __float_as_int(vh4.x); vh.oz = vh4.y; vh.cp = vh4.z; vh.sp = vh4.w;
+    const int n = vh.n & 0x7ffff, rmin = (int)((uint32_t)vh.n >> 19);
+    if (threadIdx.x == 0 && n > 0) {
+        const uint32_t ns = (uint32_t)min(n, ra.scap);       // entries beyond scap are read from global memory
+        mbar_expect_tx(bar, ns * 64u);
+        bulk_g2s(s_geo, ra.geo + (size_t)view * ra.cap, ns * 48u, bar);
+        bulk_g2s(s_aux, ra.aux + (size_t)view * ra.cap, ns * 16u, bar);
+    }
+    // row table (contract C3-C4), overlapped with the bulk copies
     for (int i = threadIdx.x; i < H; i += blockDim.x) {
         const float v = c_mul(c_sub(1.0f, c_mul(c_add((float)i, 0.5f), ra.two_over_H)), ra.tv);
         const float dz = c_fma(v, vh.cp, vh.sp);

@@ -689,6 +689,20 @@ static int render_device(gp_ctx *c, int world_begin, int n_worlds, int H, int W,
         ra.o_rgb = d_rgb ? d_rgb + v0 * 3 * HW : nullptr;
         {
             LaunchTimer lt(c, GP_KERNEL_RENDER, stream);
+#if GP_PDL
+            if (variant == GP_VARIANT_RAY && n_chunks == 1) {
+                // programmatic dependent launch on the cull enqueued just before: the render CTAs may become resident and
+                // run their view-independent prologue while the cull's last CTAs finish (griddepcontrol.wait in k_render)
+                cudaLaunchConfig_t cfg = {};
+                cfg.gridDim = dim3((unsigned)(nv * ctas_per_view)); cfg.blockDim = dim3(block);
+                cfg.dynamicSmemBytes = smem; cfg.stream = stream;
+                cudaLaunchAttribute at[1];
+                at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+                at[0].val.programmaticStreamSerializationAllowed = 1;
+                cfg.attrs = at; cfg.numAttrs = 1;
+                CK(cudaLaunchKernelEx(&cfg, fn, sc, ra));
+            } else
+#endif
             fn<<<dim3((unsigned)(nv * ctas_per_view)), dim3(block), smem, stream>>>(sc, ra);
         }
         c->launches += 1;
