@@ -48,6 +48,8 @@ def parse():
     ap.add_argument("--variant", type=int, default=-1, help="GP_OPT_VARIANT: 0 ray strips, 1 raster tiles, -1 library default")
     ap.add_argument("--tile-px", type=int, default=0, help="GP_OPT_TILE_PX override (0 = library default)")
     ap.add_argument("--pipeline", type=int, default=0, help="GP_OPT_PIPELINE override (0 = library default = 1 = serial)")
+    ap.add_argument("--t-max", type=float, default=0.0,
+                    help="override the far plane (m); 0.01 empties every list: the floor of the render pass (diagnostic, not a bench config)")
     ap.add_argument("--chunk-worlds", type=int, default=0,
                     help="worlds per gp_render_batch call (0 = as many as keep the planes under 40 GB)")
     ap.add_argument("--graph", action="store_true",
@@ -123,6 +125,8 @@ def workload_cfg(args):
         cfg = cfg.replace(H=args.res, W=args.res)
     if args.hw:
         cfg = cfg.replace(H=args.hw[0], W=args.hw[1])
+    if getattr(args, "t_max", 0.0) > 0.0:
+        cfg = cfg.replace(t_max=args.t_max)
     return cfg
 
 
@@ -133,6 +137,8 @@ def config_dict(cfg, extra=None):
         "views_per_step": cfg.views, "pixels_per_step": cfg.views * cfg.H * cfg.W,
         "worlds_per_render_call": (extra or {}).get("worlds_per_render_call", cfg.n_worlds),
         "l2": "outputs per step (%.2f GB) far exceed the 126 MB L2; no explicit flush" % (cfg.views * cfg.H * cfg.W * 12 / 1e9)}
+    if cfg.t_max != gs.config(cfg.name).t_max:
+        d["diagnostic"] = "far plane overridden to %g m (--t-max): NOT a BASELINE.json configuration" % cfg.t_max
     if extra:
         d.update(extra)
     return d

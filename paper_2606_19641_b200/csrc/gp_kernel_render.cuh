@@ -672,15 +672,18 @@ k_render(SceneConst sc, RenderArgs ra) {
                 }
             } else {
                 // any W: the strip is SR*W consecutive pixels (a multiple of 4, start 4-aligned); a lane's
-                // 4 pixels straddle two rows only when W % 4 != 0
+                // 4 pixels straddle two rows only when W % 4 != 0, and then every lane takes the per-pixel-row form: a warp
+                // in which one lane straddles would otherwise run both forms (210 x 126: 4.17 -> 4.05 ms)
                 int row = row0 + lane_row, col = lane_col, off = 0;
                 while (row <= row1) {
-                    if (col + 4 <= W)
+                    if ((W & 3) == 0)
                         resolve_quad(s_row[row].w, s_bg, kq ? kq + off : nullptr, wtab, pc + off, pi + off, pd + off,
                                      pr ? pr + off : nullptr, HW);
-                    else
-                        resolve_quad_split(s_row[row].w, s_row[row + 1].w, W - col, s_bg, kq ? kq + off : nullptr, wtab,
+                    else {      // one code path for the warp: nsplit = 4 for the lanes that do not straddle
+                        const int nsplit = min(4, W - col);
+                        resolve_quad_split(s_row[row].w, s_row[row + (nsplit < 4)].w, nsplit, s_bg, kq ? kq + off : nullptr, wtab,
                                            pc + off, pi + off, pd + off, pr ? pr + off : nullptr, HW);
+                    }
                     off += 128; row += step_row; col += step_col;
                     if (col >= W) { col -= W; ++row; }
                 }
