@@ -226,6 +226,11 @@ k_cull(SceneConst sc, CullArgs ca) {
     // grid's CTAs drain; it waits (griddepcontrol.wait) for this grid to complete before it reads the lists
     asm volatile("griddepcontrol.launch_dependents;");
 #endif
+#if GP_PDL
+    // ... and this grid may itself have been started early, behind a pose update (k_agents_update / k_dynamics_step): wait
+    // for it before the first read of a record (returns at once after a normal launch)
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+#endif
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int wl = blockIdx.x / ca.groups_per_world;                    // world within the rendered range
     const int v = (blockIdx.x - wl * ca.groups_per_world) * kCullWarps + warp;   // view within the world

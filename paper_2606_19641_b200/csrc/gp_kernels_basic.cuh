@@ -34,6 +34,9 @@ __global__ void k_prim_meta(SceneConst sc, const gp_prim *__restrict__ prims, Pr
 // a0: pose[Wn][A][4] = (cx, cy, cos, sin) -> agent records + their shading table.
 __global__ void k_agents_update(SceneConst sc, const float4 *__restrict__ pose, gp_prim *__restrict__ prims,
                                 PrimMeta *__restrict__ meta) {
+    // a cull launched behind this kernel with programmatic stream serialisation may become resident now (it waits for
+    // this grid to complete before it reads a record)
+    asm volatile("griddepcontrol.launch_dependents;");
     size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     size_t n = (size_t)sc.Wn * sc.A;
     if (i >= n) return;

@@ -635,6 +635,17 @@ static int render_device(gp_ctx *c, int world_begin, int n_worlds, int H, int W,
         ca.hdr = c->d_hdr + v0; ca.geo = c->d_geo + v0 * c->scratch_cap; ca.aux = c->d_aux + v0 * c->scratch_cap;
         {
             LaunchTimer lt(c, GP_KERNEL_CULL, st);
+#if GP_PDL
+            if (st == stream) {        // behind whatever the caller enqueued last (usually the pose update)
+                cudaLaunchConfig_t cfg = {};
+                cfg.gridDim = dim3((unsigned)((size_t)nw * gpw)); cfg.blockDim = dim3(kCullWarps * 32); cfg.stream = st;
+                cudaLaunchAttribute at[1];
+                at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+                at[0].val.programmaticStreamSerializationAllowed = 1;
+                cfg.attrs = at; cfg.numAttrs = 1;
+                CK(cudaLaunchKernelEx(&cfg, k_cull, sc, ca));
+            } else
+#endif
             k_cull<<<(unsigned)((size_t)nw * gpw), kCullWarps * 32, 0, st>>>(sc, ca);
         }
         c->launches += 1;
