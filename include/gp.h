@@ -47,8 +47,8 @@ enum {
     GP_OPT_STATS = 2,       /* 1: count executed ray/primitive tests and listed pairs         */
     GP_OPT_TIMING = 3,      /* n > 0: bracket every n-th launch of each kernel with CUDA events
                                (gp_kernel_time); 0: off                                         */
-    GP_OPT_STAGE_CAP = 4,   /* list entries per view staged in shared memory (default 128, >= 1);
-                               longer lists read their tail from global memory                  */
+    GP_OPT_STAGE_CAP = 4,   /* list entries per view staged in shared memory (>= 1; 0 = automatic: 128, or 64 for
+                               images of up to 64 x 64); longer lists read their tail from global memory */
     GP_OPT_STRIP_PX = 5,    /* target pixels per warp strip of the render pass; 0 = automatic   */
     GP_OPT_GATHER = 6,      /* how a strip works off its list: 1 gather the overlapping entries first, one lane
                                per (flat quad, row); 0 entry by entry; -1 (default) chosen from the image size

@@ -34,7 +34,7 @@ struct gp_ctx {
     ViewHdr *d_hdr = nullptr; EntryGeo *d_geo = nullptr; EntryAux *d_aux = nullptr;
     size_t scratch_views = 0; int scratch_cap = 0;
     unsigned long long *d_stats = nullptr;
-    int opt_path = GP_PATH_FAST, opt_stats = 0, opt_timing = 0, opt_stage_cap = GP_STAGE_CAP, opt_strip_px = 0, opt_gather = -1, opt_spheres = -1;
+    int opt_path = GP_PATH_FAST, opt_stats = 0, opt_timing = 0, opt_stage_cap = 0, opt_strip_px = 0, opt_gather = -1, opt_spheres = -1;
     int opt_variant = -1, opt_tile_px = 0, opt_pipeline = 1;
     cudaStream_t aux_stream = nullptr;                           // culls of later chunks run here (render_device)
     std::vector<cudaEvent_t> pipe_ev;
@@ -182,7 +182,7 @@ extern "C" int gp_set_option(gp_ctx *c, int key, int value) {
             for (unsigned &q : c->timing_seq) q = 0;
             return GP_OK;
         case GP_OPT_STAGE_CAP:
-            if (value < 1) return GP_ERR_ARG;
+            if (value < 0) return GP_ERR_ARG;
             c->opt_stage_cap = value; return GP_OK;
         case GP_OPT_GATHER:
             if (value < -1 || value > 1) return GP_ERR_ARG;
@@ -427,7 +427,10 @@ static int check_render_args(gp_ctx *c, int world_begin, int n_worlds, int agent
 // Launch shape of the render pass for an H x W image (host logic; all thresholds measured on B200).
 struct RenderPlan { int SR, log2LC, log2W, ng, ngr, nwarps, gather, scap; uint32_t magicW; size_t smem; };
 static bool plan_render(const gp_ctx *c, const SceneConst &sc, int H, int W, RenderPlan &pl) {
-    pl.scap = std::min(sc.P, c->opt_stage_cap);
+    // List entries staged in shared memory (longer lists read their tail from global memory): 128; 64 for images of up to
+    // 64 x 64 pixels, whose CTAs are small enough for the list buffer to decide how many fit an SM (measured: small 0.1072 ->
+    // 0.1026 ms, sweep 64 x 64 0.381 -> 0.348 ms; 210 x 126 and larger lose with 64)
+    pl.scap = std::min(sc.P, c->opt_stage_cap > 0 ? c->opt_stage_cap : (long long)H * W <= 64 * 64 ? 64 : GP_STAGE_CAP);
     // rows per strip (power of two): ~512 pixels, fewer for small images so that a view still has
     // >= 8 strips to spread over its warps (a strip's entries are processed serially by one warp; measured: 64 x 64 with
     // 8 strips of 512 pixels 0.1072 ms against 0.1135 with 16 of 256 on the small configuration, equal on the sweep's)
@@ -516,7 +519,7 @@ static bool plan_raster(const gp_ctx *c, const SceneConst &sc, int H, int W, Ras
     while ((1 << log2W) < W) ++log2W;
     pl.wshift = (1 << log2W) == W ? log2W : -1;
     pl.magicW = (uint32_t)((0x100000000ull + (unsigned)W - 1) / (unsigned)W);
-    pl.scap = std::min(sc.P, c->opt_stage_cap);
+    pl.scap = std::min(sc.P, c->opt_stage_cap > 0 ? c->opt_stage_cap : GP_STAGE_CAP);
     const int groups = (TR * W + 127) / 128;
     pl.nwarps = groups >= 8 ? GP_RASTER_WARPS : groups >= 2 ? 2 : 1;
     pl.smem = 48 + (size_t)pl.scap * 64 + (size_t)TR * 16 + (size_t)((W + 3) & ~3) * 4 + (size_t)TR * W * 8;
