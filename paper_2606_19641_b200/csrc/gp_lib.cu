@@ -496,6 +496,18 @@ static bool plan_render(const gp_ctx *c, const SceneConst &sc, int H, int W, Ren
                (gather ? (size_t)nwarps * kOverlapCap * sizeof(uint16_t) : 0) + (size_t)nwarps * SR * W * 8;
         if (smem <= 227 * 1024 || nwarps == 1) break;
     }
+    // Crowded worlds (the gather mode chosen for P >= 400) are bound by instruction issue, where one more CTA per SM is worth
+    // more than a complete list stage: give up staged entries, down to 80, if that lets 8 CTAs of 4 warps fit instead of 7
+    // (each CTA costs its shared memory + 1 KB; dense 256 x 256: 30.1 KB -> 27.1 KB, 6.35 -> 6.23 ms).  Store-bound shapes
+    // lose with this (sweep 256 x 256 3.97 -> 4.00 ms), 210 x 126 too (4.14 -> 4.24 ms).
+    if (c->opt_stage_cap <= 0 && gather && sc.P >= 400 && nwarps == 4 && (smem + 1024) * 8 > 227 * 1024) {
+        const size_t budget = 227 * 1024 / 8 - 1024;
+        const size_t fixed = smem - (size_t)pl.scap * 64;
+        if (fixed + 80 * 64 <= budget) {
+            pl.scap = (int)std::min<size_t>((size_t)pl.scap, (budget - fixed) / 64);
+            smem = fixed + (size_t)pl.scap * 64;
+        }
+    }
     pl.ng = ng; pl.nwarps = nwarps; pl.gather = gather; pl.smem = smem;
     return smem <= 227 * 1024;
 }
