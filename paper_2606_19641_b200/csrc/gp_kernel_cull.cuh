@@ -17,9 +17,6 @@
 
 namespace gp {
 
-#ifndef GP_PDL
-#define GP_PDL 1
-#endif
 constexpr float kNearEps = 0.01f;      // clip plane for the projection bound, metres of planar depth
 constexpr float kNearGuard = 0.05f;    // cross-section this close to the optical centre => whole image
 

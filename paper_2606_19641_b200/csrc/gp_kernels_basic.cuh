@@ -36,7 +36,9 @@ __global__ void k_agents_update(SceneConst sc, const float4 *__restrict__ pose, 
                                 PrimMeta *__restrict__ meta) {
     // a cull launched behind this kernel with programmatic stream serialisation may become resident now (it waits for
     // this grid to complete before it reads a record)
+#if GP_PDL
     asm volatile("griddepcontrol.launch_dependents;");
+#endif
     size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     size_t n = (size_t)sc.Wn * sc.A;
     if (i >= n) return;
