@@ -482,7 +482,9 @@ def run_b200(args):
                                                  "k_render's CTA -> address mapping (one CTA per view)",
                      "algorithmic_bytes_per_launch": alg_bytes_launch, "avg_launch_ms": r_avg_ms,
                      "launches_per_step": render_launches_per_step, "share_of_step": r_ms / steps_sampled / step_ms,
-                     "note": "the culls of later world chunks run concurrently with these launches on a second stream"},
+                     "note": ("GP_OPT_PIPELINE = %d: the culls of later world chunks run concurrently with these launches on a second "
+                              "stream" % args.pipeline) if args.pipeline > 1 else
+                             "one k_render launch per render call, launched with programmatic stream serialisation behind the cull"},
         "roofline_step": {"t_hbm_ms": t_hbm_ms, "t_fp32_ms": t_fp32_ms, "frac_of_slower_roof": max(t_hbm_ms, t_fp32_ms) / step_ms,
                           "executed_tests": stats["executed_tests"], "listed_pairs": stats["listed_pairs"],
                           "frac_of_write_only_roof": (alg_bytes / (wr_peak * 1e9) * 1e3 / step_ms) if wr_peak else None,
