@@ -60,6 +60,11 @@ enum {
     GP_OPT_PIPELINE = 10,   /* n >= 1 world chunks per gp_render_batch; with n > 1 the culls of chunks 1.. run on a
                                library-owned high-priority stream concurrently with the renders of earlier chunks.
                                Default 1 (serial): the overlap measured slower on every workload */
+    GP_OPT_LIST_CAP = 11,   /* n > 0: the per-view lists of the cull hold at most min(n, primitives per world) entries, so the
+                               library-owned scratch is views x n x 64 B instead of views x P x 64 B (worlds with thousands of
+                               static segments of which a view sees few).  A view whose list does not fit is rendered by the
+                               brute-force kernel in a repair pass after the render pass: results are unchanged, that view is
+                               slow.  0 (default): n = P, no repair pass.  Set before gp_reserve / the first render */
     GP_OPT_SPHERES = 7      /* are records with shape == GP_SHAPE_SPHERE drawn?  -1 (default) automatic: yes iff the
                                uploaded scene held a sphere or gp_statics_update has run since the upload (its
                                records are device memory the host never inspects); 1 yes; 0 no: sphere records

@@ -201,7 +201,8 @@ struct CullArgs {
     float msc;                         // 2 + th + tv
     float inv_th, inv_tv, halfW, halfH;
     float far_lim;                     // t_max (1 + 1e-6)
-    ViewHdr *hdr; EntryGeo *geo; EntryAux *aux; int cap;
+    ViewHdr *hdr; EntryGeo *geo; EntryAux *aux; int cap;           // cap: list stride and capacity (entries per view)
+    uint8_t *ovf;                      // non-null when cap < P: ovf[view] = 1 if the view's list did not fit
     unsigned long long *stats;
 };
 
@@ -211,6 +212,8 @@ struct CullArgs {
 #ifndef GP_CULL_MIN_CTAS
 #define GP_CULL_MIN_CTAS 4
 #endif
+// CAPPED: the lists hold fewer than P entries (GP_OPT_LIST_CAP): overflow is checked and flagged.
+template <bool CAPPED>
 __global__ void __launch_bounds__(kCullWarps * 32, GP_CULL_MIN_CTAS)
 k_cull(SceneConst sc, CullArgs ca) {
     __shared__ float4 s_p0[kCullChunk], s_p1[kCullChunk];
@@ -371,8 +374,10 @@ k_cull(SceneConst sc, CullArgs ca) {
         const unsigned kmask = __ballot_sync(0xffffffffu, keep);
         if (keep) {
             const int slot = cnt + __popc(kmask & lt_mask);
-            vgeo[slot] = g;
-            vaux[slot] = x;
+            if (!CAPPED || slot < ca.cap) {
+                vgeo[slot] = g;
+                vaux[slot] = x;
+            }
         }
         cnt += __popc(kmask);
         }
@@ -381,7 +386,9 @@ k_cull(SceneConst sc, CullArgs ca) {
     if (!active) return;
     rmin = __reduce_min_sync(0xffffffffu, rmin);
     if (lane == 0) {
-        ViewHdr h; h.n = cnt | (rmin << 19); h.oz = cam.oz; h.cp = cam.cp; h.sp = cam.sp;
+        const bool over = CAPPED && cnt > ca.cap; // the list did not fit: draw nothing here, the brute-force repair pass
+        if (over) ca.ovf[view] = 1;               // renders this view from the records
+        ViewHdr h; h.n = over ? (0x1fff << 19) : (cnt | (rmin << 19)); h.oz = cam.oz; h.cp = cam.cp; h.sp = cam.sp;
         ca.hdr[view] = h;
         if (ca.stats) atomicAdd(&ca.stats[1], (unsigned long long)cnt);
     }

@@ -100,8 +100,9 @@ __global__ void __launch_bounds__(256)
 k_render_brute(SceneConst sc, const gp_prim *__restrict__ prims, const float2 *__restrict__ pitch,
                int world_begin, int H, int W, float th, float tv,
                uint8_t *__restrict__ o_cls, int32_t *__restrict__ o_inst, float *__restrict__ o_depth,
-               uint8_t *__restrict__ o_rgb) {
+               uint8_t *__restrict__ o_rgb, const uint8_t *__restrict__ only_flagged) {
     const int view = blockIdx.x;
+    if (only_flagged && !only_flagged[view]) return;    // repair pass of a capped list (GP_OPT_LIST_CAP): flagged views only
     const int va = view / sc.C, cam = view - va * sc.C;
     const int w = world_begin + va / sc.A, a = va % sc.A;
     const gp_prim *wp = prims + (size_t)w * sc.P;

@@ -32,10 +32,11 @@ struct gp_ctx {
     gp_prim *h_stage = nullptr; size_t h_stage_bytes = 0;        // pinned upload staging
     // per-view scratch of the fast path
     ViewHdr *d_hdr = nullptr; EntryGeo *d_geo = nullptr; EntryAux *d_aux = nullptr;
+    uint8_t *d_ovf = nullptr;                                    // per view: its list did not fit GP_OPT_LIST_CAP
     size_t scratch_views = 0; int scratch_cap = 0;
     unsigned long long *d_stats = nullptr;
     int opt_path = GP_PATH_FAST, opt_stats = 0, opt_timing = 0, opt_stage_cap = 0, opt_strip_px = 0, opt_gather = -1, opt_spheres = -1;
-    int opt_variant = -1, opt_tile_px = 0, opt_pipeline = 1;
+    int opt_variant = -1, opt_tile_px = 0, opt_pipeline = 1, opt_list_cap = 0;
     cudaStream_t aux_stream = nullptr;                           // culls of later chunks run here (render_device)
     std::vector<cudaEvent_t> pipe_ev;
     struct Timed { int kernel; cudaEvent_t a, b; };
@@ -139,8 +140,8 @@ extern "C" int gp_create(gp_ctx **out, int cuda_device) {
 static void free_scene(gp_ctx *c) {
     cudaFree(c->d_prims); cudaFree(c->d_meta); cudaFree(c->d_pitch);
     c->d_prims = nullptr; c->d_meta = nullptr; c->d_pitch = nullptr;
-    cudaFree(c->d_hdr); cudaFree(c->d_geo); cudaFree(c->d_aux);
-    c->d_hdr = nullptr; c->d_geo = nullptr; c->d_aux = nullptr; c->scratch_views = 0; c->scratch_cap = 0;
+    cudaFree(c->d_hdr); cudaFree(c->d_geo); cudaFree(c->d_aux); cudaFree(c->d_ovf);
+    c->d_hdr = nullptr; c->d_geo = nullptr; c->d_aux = nullptr; c->d_ovf = nullptr; c->scratch_views = 0; c->scratch_cap = 0;
     cudaFree(c->d_pose); c->d_pose = nullptr;
     c->have_scene = false;
 }
@@ -199,6 +200,9 @@ extern "C" int gp_set_option(gp_ctx *c, int key, int value) {
         case GP_OPT_SPHERES:
             if (value < -1 || value > 1) return GP_ERR_ARG;
             c->opt_spheres = value; return GP_OK;
+        case GP_OPT_LIST_CAP:
+            if (value < 0) return GP_ERR_ARG;
+            c->opt_list_cap = value; return GP_OK;
         case GP_OPT_STRIP_PX:
             if (value < 0 || value > 4096) return GP_ERR_ARG;
             c->opt_strip_px = value; return GP_OK;
@@ -397,18 +401,25 @@ extern "C" int gp_camera_rig_set(gp_ctx *c, int n_cams, const gp_camera *h_rig) 
     return GP_OK;
 }
 
+// Per-view scratch of the fast path: header + list of up to `cap` entries per view, cap = P (every primitive of the world could be
+// listed) unless GP_OPT_LIST_CAP sets a smaller one; then a view whose list does not fit is flagged in d_ovf and rendered by
+// the brute-force kernel after the render pass (render_device), so the result stays the all-primitive definition.
+static int list_cap(const gp_ctx *c) {
+    return c->opt_list_cap > 0 ? std::min(c->sc.P, c->opt_list_cap) : c->sc.P;
+}
 static int ensure_scratch(gp_ctx *c, size_t views) {
-    const int cap = c->sc.P;
+    const int cap = list_cap(c);
     if (c->scratch_views >= views && c->scratch_cap == cap) return GP_OK;
     CK(cudaDeviceSynchronize());
-    cudaFree(c->d_hdr); cudaFree(c->d_geo); cudaFree(c->d_aux);
-    c->d_hdr = nullptr; c->d_geo = nullptr; c->d_aux = nullptr; c->scratch_views = 0;
+    cudaFree(c->d_hdr); cudaFree(c->d_geo); cudaFree(c->d_aux); cudaFree(c->d_ovf);
+    c->d_hdr = nullptr; c->d_geo = nullptr; c->d_aux = nullptr; c->d_ovf = nullptr; c->scratch_views = 0;
     if (cudaMalloc(&c->d_hdr, views * sizeof(ViewHdr)) != cudaSuccess ||
         cudaMalloc(&c->d_geo, views * cap * sizeof(EntryGeo)) != cudaSuccess ||
-        cudaMalloc(&c->d_aux, views * cap * sizeof(EntryAux)) != cudaSuccess) {
+        cudaMalloc(&c->d_aux, views * cap * sizeof(EntryAux)) != cudaSuccess ||
+        cudaMalloc(&c->d_ovf, views) != cudaSuccess) {
         cudaGetLastError();
-        cudaFree(c->d_hdr); cudaFree(c->d_geo); cudaFree(c->d_aux);
-        c->d_hdr = nullptr; c->d_geo = nullptr; c->d_aux = nullptr;
+        cudaFree(c->d_hdr); cudaFree(c->d_geo); cudaFree(c->d_aux); cudaFree(c->d_ovf);
+        c->d_hdr = nullptr; c->d_geo = nullptr; c->d_aux = nullptr; c->d_ovf = nullptr;
         return GP_ERR_NOMEM;
     }
     c->scratch_views = views; c->scratch_cap = cap;
@@ -599,7 +610,7 @@ static int render_device(gp_ctx *c, int world_begin, int n_worlds, int H, int W,
         {
             LaunchTimer lt(c, GP_KERNEL_BRUTE, stream);
             k_render_brute<<<grid, 256, 0, stream>>>(sc, c->d_prims, c->d_pitch, world_begin, H, W, th, tv,
-                                                      d_class, d_instance, d_depth, d_rgb);
+                                                      d_class, d_instance, d_depth, d_rgb, nullptr);
         }
         c->launches += 1;
         CK(cudaGetLastError());
@@ -643,12 +654,14 @@ static int render_device(gp_ctx *c, int world_begin, int n_worlds, int H, int W,
     cargs.inv_th = 1.0f / th; cargs.inv_tv = 1.0f / tv; cargs.halfW = 0.5f * (float)W; cargs.halfH = 0.5f * (float)H;
     cargs.far_lim = sc.t_max * (1.0f + 1e-6f);
     cargs.cap = c->scratch_cap; cargs.stats = stats;
+    const bool capped = c->scratch_cap < sc.P;                         // lists may overflow: flag + brute-force repair pass
     auto launch_cull = [&](int ci, cudaStream_t st) -> int {
         const int w0 = ci * wpc, nw = std::min(wpc, n_worlds - w0);
         const size_t v0 = (size_t)w0 * vpw;
         CullArgs ca = cargs;
         ca.world_begin = world_begin + w0;
         ca.hdr = c->d_hdr + v0; ca.geo = c->d_geo + v0 * c->scratch_cap; ca.aux = c->d_aux + v0 * c->scratch_cap;
+        ca.ovf = capped ? c->d_ovf + v0 : nullptr;
         {
             LaunchTimer lt(c, GP_KERNEL_CULL, st);
 #if GP_PDL
@@ -659,10 +672,11 @@ static int render_device(gp_ctx *c, int world_begin, int n_worlds, int H, int W,
                 at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
                 at[0].val.programmaticStreamSerializationAllowed = 1;
                 cfg.attrs = at; cfg.numAttrs = 1;
-                CK(cudaLaunchKernelEx(&cfg, k_cull, sc, ca));
+                CK(cudaLaunchKernelEx(&cfg, capped ? k_cull<true> : k_cull<false>, sc, ca));
             } else
 #endif
-            k_cull<<<(unsigned)((size_t)nw * gpw), kCullWarps * 32, 0, st>>>(sc, ca);
+            if (capped) k_cull<true><<<(unsigned)((size_t)nw * gpw), kCullWarps * 32, 0, st>>>(sc, ca);
+            else k_cull<false><<<(unsigned)((size_t)nw * gpw), kCullWarps * 32, 0, st>>>(sc, ca);
         }
         c->launches += 1;
         CK(cudaGetLastError());
@@ -699,6 +713,7 @@ static int render_device(gp_ctx *c, int world_begin, int n_worlds, int H, int W,
         ra.magic_vpw = (uint32_t)(((1ull << (31 + L)) + (unsigned)vpw - 1) / (unsigned)vpw);
     }
     const size_t HW = (size_t)H * W;
+    if (capped) CK(cudaMemsetAsync(c->d_ovf, 0, views, stream));
     rc = launch_cull(0, stream);                                       // chunk 0: nothing to overlap with yet
     if (rc != GP_OK) return rc;
     for (int ci = 1; ci < n_chunks; ++ci) {                            // the other culls run ahead on the side stream
@@ -731,6 +746,17 @@ static int render_device(gp_ctx *c, int world_begin, int n_worlds, int H, int W,
             } else
 #endif
             fn<<<dim3((unsigned)(nv * ctas_per_view)), dim3(block), smem, stream>>>(sc, ra);
+        }
+        c->launches += 1;
+        CK(cudaGetLastError());
+    }
+    if (capped) {
+        // repair pass: the views whose list overflowed the cap (the render pass drew only the background for them) are
+        // rendered by the brute-force kernel, one CTA per flagged view; the CTAs of all other views exit at once
+        {
+            LaunchTimer lt(c, GP_KERNEL_BRUTE, stream);
+            k_render_brute<<<dim3((unsigned)views, 1), 256, 0, stream>>>(sc, c->d_prims, c->d_pitch, world_begin, H, W, th, tv,
+                                                                           d_class, d_instance, d_depth, d_rgb, c->d_ovf);
         }
         c->launches += 1;
         CK(cudaGetLastError());

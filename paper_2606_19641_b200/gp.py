@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(_HERE, "libgp.so")
 GP_OK, GP_ERR_ARG, GP_ERR_ALIGN, GP_ERR_STATE, GP_ERR_RANGE, GP_ERR_CUDA, GP_ERR_ARCH, GP_ERR_NOMEM = \
     0, -1, -2, -3, -4, -5, -6, -7
 GP_OPT_PATH, GP_OPT_STATS, GP_OPT_TIMING, GP_OPT_STAGE_CAP, GP_OPT_STRIP_PX, GP_OPT_GATHER, GP_OPT_SPHERES = 1, 2, 3, 4, 5, 6, 7
-GP_OPT_VARIANT, GP_OPT_TILE_PX, GP_OPT_PIPELINE = 8, 9, 10
+GP_OPT_VARIANT, GP_OPT_TILE_PX, GP_OPT_PIPELINE, GP_OPT_LIST_CAP = 8, 9, 10, 11
 GP_VARIANT_RAY, GP_VARIANT_RASTER = 0, 1
 GP_KERNEL_UPDATE, GP_KERNEL_CULL, GP_KERNEL_RENDER, GP_KERNEL_BRUTE, GP_KERNEL_DYNAMICS, GP_KERNEL_OBSERVE = 0, 1, 2, 3, 4, 5
 GP_PATH_FAST, GP_PATH_BRUTE = 0, 1
