@@ -311,6 +311,20 @@ def run_b200(args):
     r.set_option(gp.GP_OPT_TIMING, 0)
     ms = shard.max_over_ranks(ms, dev)
 
+    # per-step distribution ("the per-frame distribution"): a separate pass after the timed region, every step
+    # bracketed by its own pair of events (which spaces the launches a little: the headline stays the back-to-back figure)
+    n_dist = min(args.steps, 256)
+    evs = [torch.cuda.Event(enable_timing=True) for _ in range(n_dist + 1)]
+    torch.cuda.synchronize()
+    evs[0].record()
+    for q in range(n_dist):
+        step(args.warmup + q)
+        evs[q + 1].record()
+    torch.cuda.synchronize()
+    per_step = sorted(evs[q].elapsed_time(evs[q + 1]) for q in range(n_dist))
+    step_dist = {"n": n_dist, "min": per_step[0], "median": per_step[n_dist // 2], "p95": per_step[min(n_dist - 1, (n_dist * 95) // 100)],
+                 "max": per_step[-1], "unit": "ms", "how": "one CUDA-event pair per step, separate pass after the timed region"}
+
     # one instrumented frame (not timed): executed tests and listed pairs for the FP32 roof
     r.set_option(gp.GP_OPT_STATS, 1)
     stats = {}
@@ -473,6 +487,7 @@ def run_b200(args):
         "kernels_ms_per_step": {k: v[0] / steps_sampled for k, v in ktimes.items()},
         "kernel_samples": {k: int(v[1]) for k, v in ktimes.items()},
         "cuda_graph": bool(graphs),
+        "step_ms_distribution": step_dist,
         "roofline": {"bound": "hbm", "kernel": "k_render", "achieved": achieved, "peak": peak, "unit": "GB/s",
                      "frac": achieved / peak, "traffic": traffic, "traffic_source": traffic_source, "peak_source": peak_src,
                      "peak_write_only": wr_peak, "frac_write_only": (achieved / wr_peak) if wr_peak else None,
