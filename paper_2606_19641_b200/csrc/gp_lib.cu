@@ -17,6 +17,9 @@
 
 using namespace gp;
 
+#ifndef GP_TINY_PX
+#define GP_TINY_PX 1024            // images of up to this many pixels are rendered by one-warp CTAs (plan_render)
+#endif
 #ifndef GP_STAGE_CAP
 #define GP_STAGE_CAP 128
 #endif
@@ -441,12 +444,18 @@ static bool plan_render(const gp_ctx *c, const SceneConst &sc, int H, int W, Ren
     // List entries staged in shared memory (longer lists read their tail from global memory): 128; 64 for images of up to
     // 64 x 64 pixels, whose CTAs are small enough for the list buffer to decide how many fit an SM (measured: small 0.1072 ->
     // 0.1026 ms, sweep 64 x 64 0.381 -> 0.348 ms; 210 x 126 and larger lose with 64)
-    pl.scap = std::min(sc.P, c->opt_stage_cap > 0 ? c->opt_stage_cap : (long long)H * W <= 64 * 64 ? 64 : GP_STAGE_CAP);
+    // (48 for images of up to 32 x 32, rendered by one-warp CTAs of which 32 then fit an SM)
+    const bool tiny = (long long)H * W <= GP_TINY_PX;
+    pl.scap = std::min(sc.P, c->opt_stage_cap > 0 ? c->opt_stage_cap : tiny ? 48 : (long long)H * W <= 64 * 64 ? 64 : GP_STAGE_CAP);
     // rows per strip (power of two): ~512 pixels, fewer for small images so that a view still has
     // >= 8 strips to spread over its warps (a strip's entries are processed serially by one warp; measured: 64 x 64 with
     // 8 strips of 512 pixels 0.1072 ms against 0.1135 with 16 of 256 on the small configuration, equal on the sweep's)
     int strip_px = c->opt_strip_px;
     if (strip_px <= 0) { strip_px = 512; while (strip_px > 128 && H * W / strip_px < 8) strip_px /= 2; }
+    // Images of up to 32 x 32: ONE warp per view and strips of 256 pixels (measured on the sweep's 32 x 32: 0.148 ms against
+    // 0.166 with 2 warps and 128-pixel strips, 0.188 with 1 warp and 128, 0.157 with 1 warp and 512) — a view of 1024 pixels is
+    // too little work to share: the second warp costs a barrier, a strip counter and its share of per-strip list scans
+    if (tiny && c->opt_strip_px <= 0) strip_px = std::max(strip_px, 256);
     const int align = (W & 1) ? 4 : (W & 2) ? 2 : 1;           // strips start on a multiple of 4 pixels
     int SR = align;
     while (SR < 16 && SR * 2 * W <= strip_px) SR *= 2;
@@ -492,7 +501,7 @@ static bool plan_render(const gp_ctx *c, const SceneConst &sc, int H, int W, Ren
     // warps per CTA (= per view): 4; 2 for images of up to 64 x 64 pixels, where twice as many (shorter-lived) CTAs
     // per SM hide the per-view prologue better (32 x 32: 0.230 -> 0.174 ms, 64 x 64: 0.457 -> 0.384 ms; measured slower
     // from 128 x 128 up)
-    const int max_warps = (long long)H * W <= 64 * 64 ? (GP_RENDER_WARPS < 2 ? GP_RENDER_WARPS : 2) : GP_RENDER_WARPS;
+    const int max_warps = tiny ? 1 : (long long)H * W <= 64 * 64 ? (GP_RENDER_WARPS < 2 ? GP_RENDER_WARPS : 2) : GP_RENDER_WARPS;
     int nwarps = n_strips < max_warps ? n_strips : max_warps;
     // List handling (measured on B200): gathering pays when many entries meet a strip — small images
     // (the same list over fewer pixels) or crowded worlds; entry-by-entry is ~1 % faster on the store-bound cases.
