@@ -38,7 +38,8 @@ enum {
     GP_ERR_RANGE = -4,      /* world range outside the scene, agents != agents_per_world     */
     GP_ERR_CUDA = -5,       /* a CUDA runtime call failed (text via gp_error_string)         */
     GP_ERR_ARCH = -6,       /* the device is not compute capability 10.x                     */
-    GP_ERR_NOMEM = -7       /* device or host allocation failed                              */
+    GP_ERR_NOMEM = -7,      /* device or host allocation failed                              */
+    GP_ERR_LIMIT = -8       /* gp_render_static: scene or image larger than its fixed scratch */
 };
 
 /* gp_set_option keys */
@@ -201,6 +202,59 @@ int gp_render_batch(gp_ctx *ctx, int world_begin, int n_worlds, int agents, int 
  * Synchronises the device if it has to grow the scratch.  Call it again after gp_camera_rig_set changed the number of
  * cameras.  GP_ERR_STATE before gp_scene_upload, GP_ERR_RANGE if n_worlds exceeds the scene, GP_ERR_NOMEM. */
 int gp_reserve(gp_ctx *ctx, int n_worlds, int H, int W);
+
+/* ---- rendering without any allocation ----------------------------------------------------------------------------
+ *
+ * Who this is for.  Every other render call needs a gp_ctx, and a gp_ctx owns device memory that the library takes from
+ * cudaMalloc (gp_create, gp_scene_upload, the first gp_render_batch of a shape).  Some users of a simulator step cannot
+ * accept that:
+ *   - a training process whose framework has already claimed all of HBM for its own pool (a caching allocator that grew to
+ *     the card's limit, or one told to pre-reserve it): a cudaMalloc from a third-party library then simply fails;
+ *   - a latency-bound actor or evaluation loop: cudaMalloc and cudaFree stall the whole device while they run, so one late
+ *     allocation in the renderer shows up as a hitch in every other stream of the process;
+ *   - a deployment that accounts for each byte of device memory up front and forbids libraries from allocating behind it.
+ * gp_render_static serves those.  It takes the scene as device memory the caller already has, renders every view of it
+ * (steps a1-a9, the default front camera) into caller-owned planes, and keeps its intermediates - the shading table, the
+ * view headers and the per-view primitive lists that the cull writes and the render pass reads - in one fixed array that is
+ * part of the library image.  It never calls cudaMalloc, cudaFree or any routine that allocates, and it creates no context.
+ *
+ * The price is a fixed size.  The array is 9 535 488 bytes (about 9.1 MiB) and exists on every GPU of a process that loads
+ * libgp.so, from load until exit, whether this function is called or not.  It bounds the scene:
+ *     views   = n_worlds * agents_per_world                      <= GP_STATIC_MAX_VIEWS
+ *     records = n_worlds * (agents_per_world + quads_per_world)  <= GP_STATIC_MAX_PRIMS
+ *     slots   = views * (agents_per_world + quads_per_world)     <= GP_STATIC_MAX_ENTRIES
+ * (16 worlds x 32 agents + 120 quads, or 4 worlds of the paper-scale shape, fit).  Anything larger is refused with
+ * GP_ERR_LIMIT before a single launch; split the scene by worlds or use a gp_ctx.
+ *
+ * Arguments
+ *   cuda_device  the device d_prims and the planes live on; must be sm_100 (GP_ERR_ARCH)
+ *   desc         HOST, read before the call returns.  n_worlds, agents_per_world, quads_per_world and the constants as for
+ *                gp_scene_upload
+ *   d_prims      DEVICE [n_worlds][agents_per_world + quads_per_world] gp_prim, 16-byte aligned, agents first in each
+ *                world.  Read only; NOT validated (the host never sees it): cls is masked to 0..7 and spheres are drawn
+ *   d_pitch_cs   DEVICE [n_worlds][agents_per_world][2] = (cos p, sin p), 8-byte aligned, or NULL for pitch 0
+ *   H, W, fov_rad, d_class, d_instance, d_depth, d_rgb   exactly as for gp_render_batch, with one restriction: only image
+ *                sizes of the fast path (W >= 4, (H * W) % 4 == 0, one strip within shared memory); others are GP_ERR_ARG
+ * The result is the same, bit for bit, as gp_scene_upload + gp_cameras_set + gp_render_batch on the same records.
+ *
+ * Rules of use
+ *   - The first call on each device does a one-off set-up with that device current: it asks the runtime where the array
+ *     lives on that device and checks the architecture.  Make that first call outside any stream capture, and before the
+ *     part of the program that must not be disturbed.
+ *   - All calls on one device share the one array, and it keeps what the previous call left in it.  Nothing in it has to
+ *     start at zero - every header and every list slot that is read was written earlier in the same call - and the
+ *     headers of the call's views are cleared first all the same, so stale lengths can never be picked up.  Because the
+ *     array is shared, two calls must not overlap on the GPU: issue them on one stream, or order the streams with
+ *     events.  Calls that run concurrently race on the lists and the planes of both are undefined.  The same holds for
+ *     two host threads calling at once on one device.
+ *   - Work is enqueued on `stream`; the call does not synchronise.
+ * Errors: GP_ERR_ARG, GP_ERR_ALIGN, GP_ERR_LIMIT, GP_ERR_ARCH, GP_ERR_CUDA; all but the last write nothing. */
+#define GP_STATIC_MAX_VIEWS   4096
+#define GP_STATIC_MAX_PRIMS   32768
+#define GP_STATIC_MAX_ENTRIES 131072
+int gp_render_static(int cuda_device, const gp_scene_desc *desc, const gp_prim *d_prims, const float *d_pitch_cs,
+                     int H, int W, float fov_rad, uint8_t *d_class, int32_t *d_instance, float *d_depth,
+                     uint8_t *d_rgb, void *stream);
 
 /* End-to-end variant with HOST buffers: copies h_pose (HOST [Wn][A][4], may be NULL = keep poses) to the
  * device, updates the agents, renders worlds [world_begin, world_begin+n_worlds) in chunks through

@@ -4,6 +4,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -114,6 +115,8 @@ extern "C" const char *gp_error_string(int code) {
         case GP_ERR_CUDA: return g_cuda_msg;
         case GP_ERR_ARCH: return "device is not sm_100 (B200); no fallback path exists";
         case GP_ERR_NOMEM: return "out of memory";
+        case GP_ERR_LIMIT: return "gp_render_static: the scene exceeds GP_STATIC_MAX_VIEWS / _PRIMS / _ENTRIES (its scratch "
+                                  "is a fixed array; render fewer worlds per call or use a gp_ctx)";
         default: return "unknown error code";
     }
 }
@@ -955,5 +958,133 @@ extern "C" int gp_kernel_time(gp_ctx *c, int kernel, double *total_ms, uint64_t 
 extern "C" int gp_launch_count(gp_ctx *c, uint64_t *launches) {
     if (!c || !launches) return GP_ERR_ARG;
     *launches = c->launches;
+    return GP_OK;
+}
+
+// ---- gp_render_static: the render step for callers that must not allocate (include/gp.h) ---------------------------
+//
+// Some processes cannot let this library call cudaMalloc: the training framework already owns all of HBM, or the loop
+// cannot afford the device-wide stall of an allocation, or device memory is budgeted to the byte.  For them the
+// intermediates of cull + render live in the fixed array below instead of a gp_ctx.  The array is part of the library
+// image: every GPU of a process that loads libgp.so carries its kStBytes from load to exit.  Sections (each starts on a
+// multiple of 256 bytes):
+namespace {
+constexpr size_t kStHdr = 0;                                                               // ViewHdr  [MAX_VIEWS]
+constexpr size_t kStPitch = kStHdr + (size_t)GP_STATIC_MAX_VIEWS * sizeof(ViewHdr);       // float2   [MAX_VIEWS]   (pitch 0)
+constexpr size_t kStMeta = kStPitch + (size_t)GP_STATIC_MAX_VIEWS * sizeof(float2);       // PrimMeta [MAX_PRIMS]
+constexpr size_t kStGeo = kStMeta + (size_t)GP_STATIC_MAX_PRIMS * sizeof(PrimMeta);       // EntryGeo [MAX_ENTRIES]
+constexpr size_t kStAux = kStGeo + (size_t)GP_STATIC_MAX_ENTRIES * sizeof(EntryGeo);      // EntryAux [MAX_ENTRIES]
+constexpr size_t kStBytes = kStAux + (size_t)GP_STATIC_MAX_ENTRIES * sizeof(EntryAux);
+static_assert(kStPitch % 256 == 0 && kStMeta % 256 == 0 && kStGeo % 256 == 0 && kStAux % 256 == 0, "section alignment");
+static_assert(kStBytes == 9535488, "include/gp.h states this size");
+constexpr int kStMaxDevices = 64;
+}  // namespace
+
+static __device__ __align__(256) unsigned char g_static_scratch[kStBytes];
+
+// In host code `g_static_scratch` is only a handle for the runtime, not an address a kernel could use: the address on
+// each device comes from cudaGetSymbolAddress, asked once per device with that device current, and is kept here.
+static std::mutex g_static_mu;
+static unsigned char *g_static_base[kStMaxDevices];
+
+static int static_scratch_base(int dev, unsigned char **base) {      // the caller has made `dev` current
+    std::lock_guard<std::mutex> lock(g_static_mu);
+    if (!g_static_base[dev]) {
+        int major = 0;
+        CK(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
+        if (major != 10) return GP_ERR_ARCH;
+        unsigned char *p = nullptr;
+        CK(cudaGetSymbolAddress(reinterpret_cast<void **>(&p), g_static_scratch));
+        if (!p || (reinterpret_cast<uintptr_t>(p) & 255u)) return cuda_fail(cudaErrorInvalidSymbol, "cudaGetSymbolAddress(g_static_scratch)");
+        g_static_base[dev] = p;
+    }
+    *base = g_static_base[dev];
+    return GP_OK;
+}
+
+extern "C" int gp_render_static(int cuda_device, const gp_scene_desc *d, const gp_prim *d_prims, const float *d_pitch_cs,
+                                int H, int W, float fov_rad, uint8_t *d_class, int32_t *d_instance, float *d_depth,
+                                uint8_t *d_rgb, void *stream_) {
+    if (!d || !d_prims || !d_class || !d_instance || !d_depth) return GP_ERR_ARG;
+    if (cuda_device < 0 || cuda_device >= kStMaxDevices) return GP_ERR_ARG;
+    if (d->n_worlds < 1 || d->agents_per_world < 1 || d->quads_per_world < 0) return GP_ERR_ARG;
+    if (!(d->cam_height > 0.0f) || !(d->t_max > 0.0f) || !(d->ambient >= 0.0f && d->ambient <= 1.0f)) return GP_ERR_ARG;
+    if (H < 1 || W < 4 || H > 4096 || W > 4096 || (((long long)H * W) & 3)) return GP_ERR_ARG;
+    if (!(fov_rad > 0.0f && fov_rad < 3.1415f)) return GP_ERR_ARG;
+    if (!aligned16(d_prims) || !aligned16(d_class) || !aligned16(d_instance) || !aligned16(d_depth) || !aligned16(d_rgb) ||
+        (reinterpret_cast<uintptr_t>(d_pitch_cs) & 7u)) return GP_ERR_ALIGN;
+    // the fixed scratch bounds the scene: refuse anything larger before touching the device
+    const long long P = (long long)d->agents_per_world + d->quads_per_world;
+    const long long views = (long long)d->n_worlds * d->agents_per_world;
+    if (views > GP_STATIC_MAX_VIEWS || (long long)d->n_worlds * P > GP_STATIC_MAX_PRIMS || views * P > GP_STATIC_MAX_ENTRIES)
+        return GP_ERR_LIMIT;
+
+    gp_ctx plan_opts;                      // launch-shape rules of the ordinary path with every option at its default
+    plan_opts.device = cuda_device;        // (host object only: it owns no device memory and is never passed to a kernel)
+    GP_ON_DEVICE(&plan_opts);
+    unsigned char *base = nullptr;
+    int rc = static_scratch_base(cuda_device, &base);
+    if (rc != GP_OK) return rc;
+    ViewHdr *s_hdr = reinterpret_cast<ViewHdr *>(base + kStHdr);
+    float2 *s_pitch = reinterpret_cast<float2 *>(base + kStPitch);
+    PrimMeta *s_meta = reinterpret_cast<PrimMeta *>(base + kStMeta);
+    EntryGeo *s_geo = reinterpret_cast<EntryGeo *>(base + kStGeo);
+    EntryAux *s_aux = reinterpret_cast<EntryAux *>(base + kStAux);
+
+    SceneConst sc{};
+    sc.Wn = d->n_worlds; sc.A = d->agents_per_world; sc.Q = d->quads_per_world; sc.P = (int)P;
+    sc.C = 1; sc.rig[0] = make_float4(1.0f, 0.0f, 1.0f, 0.0f);            // the default rig: one front-centre camera
+    sc.spheres = 1;                                                       // the records are never seen by the host
+    sc.cam_h = d->cam_height; sc.t_max = d->t_max;
+    sc.Lx = d->light[0]; sc.Ly = d->light[1]; sc.Lz = d->light[2]; sc.ambient = d->ambient;
+    for (int k = 0; k < 8; ++k)
+        sc.pal[k] = (uint32_t)d->palette[k][0] | ((uint32_t)d->palette[k][1] << 8) | ((uint32_t)d->palette[k][2] << 16);
+    RenderPlan pl{};
+    if (!plan_render(&plan_opts, sc, H, W, pl)) return GP_ERR_ARG;       // not even one warp's strip fits shared memory
+    const RenderFn fn = kRenderFns[pl.gather][1][0][pl.ng == 4 ? 3 : pl.ng];
+    // Permit the kernel the largest dynamic shared memory there is, on every call: contexts on this device raise and lower
+    // the same attribute for their own needs, and the maximum satisfies all of them
+    CK(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+
+    cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+    const float th = (float)tan(0.5 * (double)fov_rad);                   // C2, host side
+    const float tv = th * ((float)H / (float)W);
+    const int vpw = sc.A;
+    // The array still holds the previous call's headers and lists.  Each header read below is rewritten by this call's
+    // cull first; clearing them costs 16 bytes per view and rules out a stale list length whatever else goes wrong.
+    CK(cudaMemsetAsync(s_hdr, 0, (size_t)views * sizeof(ViewHdr), stream));
+    k_prim_meta<<<(unsigned)(((size_t)sc.Wn * sc.P + 255) / 256), 256, 0, stream>>>(sc, d_prims, s_meta);
+    if (!d_pitch_cs) k_fill_pitch<<<(unsigned)((views + 255) / 256), 256, 0, stream>>>(s_pitch, (size_t)views);
+    CK(cudaGetLastError());
+
+    const int gpw = (vpw + kCullWarps - 1) / kCullWarps;
+    CullArgs ca{};
+    ca.prims = d_prims; ca.pitch = d_pitch_cs ? reinterpret_cast<const float2 *>(d_pitch_cs) : s_pitch;
+    ca.world_begin = 0; ca.groups_per_world = gpw; ca.H = H; ca.W = W; ca.th = th; ca.tv = tv;
+    ca.sth = sqrtf(fmaf(th, th, 1.0f)) * 1.0001f; ca.stv = sqrtf(fmaf(tv, tv, 1.0f)) * 1.0001f;
+    ca.msc = 2.0f + th + tv;
+    ca.inv_th = 1.0f / th; ca.inv_tv = 1.0f / tv; ca.halfW = 0.5f * (float)W; ca.halfH = 0.5f * (float)H;
+    ca.far_lim = sc.t_max * (1.0f + 1e-6f);
+    ca.hdr = s_hdr; ca.geo = s_geo; ca.aux = s_aux; ca.cap = sc.P;        // a list can hold the whole world: no overflow
+    ca.ovf = nullptr; ca.stats = nullptr;
+    k_cull<false><<<(unsigned)((size_t)sc.Wn * gpw), kCullWarps * 32, 0, stream>>>(sc, ca);
+    CK(cudaGetLastError());
+
+    RenderArgs ra{};
+    ra.hdr = s_hdr; ra.geo = s_geo; ra.aux = s_aux; ra.meta = s_meta;
+    ra.cap = sc.P; ra.scap = pl.scap; ra.world_begin = 0; ra.H = H; ra.W = W; ra.th = th; ra.tv = tv;
+    ra.SR = pl.SR; ra.log2LC = pl.log2LC; ra.log2W = pl.log2W; ra.ngr = pl.ngr; ra.magicW = pl.magicW;
+    ra.o_cls = d_class; ra.o_inst = d_instance; ra.o_depth = d_depth; ra.o_rgb = d_rgb; ra.stats = nullptr;
+    ra.n_strips = (H + pl.SR - 1) / pl.SR;
+    ra.magicSR = (uint32_t)((0x100000000ull + (unsigned)pl.SR - 1) / (unsigned)pl.SR);
+    ra.two_over_H = 2.0f / (float)H; ra.two_over_W = 2.0f / (float)W;
+    {
+        int L = 0;
+        while ((1ll << L) < vpw) ++L;
+        ra.shift_vpw = 31 + L;
+        ra.magic_vpw = (uint32_t)(((1ull << (31 + L)) + (unsigned)vpw - 1) / (unsigned)vpw);
+    }
+    fn<<<dim3((unsigned)views), dim3((unsigned)pl.nwarps * 32), pl.smem, stream>>>(sc, ra);
+    CK(cudaGetLastError());
     return GP_OK;
 }

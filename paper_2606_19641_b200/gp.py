@@ -15,6 +15,8 @@ LIB_PATH = os.path.join(_HERE, "libgp.so")
 
 GP_OK, GP_ERR_ARG, GP_ERR_ALIGN, GP_ERR_STATE, GP_ERR_RANGE, GP_ERR_CUDA, GP_ERR_ARCH, GP_ERR_NOMEM = \
     0, -1, -2, -3, -4, -5, -6, -7
+GP_ERR_LIMIT = -8
+GP_STATIC_MAX_VIEWS, GP_STATIC_MAX_PRIMS, GP_STATIC_MAX_ENTRIES = 4096, 32768, 131072
 GP_OPT_PATH, GP_OPT_STATS, GP_OPT_TIMING, GP_OPT_STAGE_CAP, GP_OPT_STRIP_PX, GP_OPT_GATHER, GP_OPT_SPHERES = 1, 2, 3, 4, 5, 6, 7
 GP_OPT_VARIANT, GP_OPT_TILE_PX, GP_OPT_PIPELINE, GP_OPT_LIST_CAP = 8, 9, 10, 11
 GP_VARIANT_RAY, GP_VARIANT_RASTER = 0, 1
@@ -25,7 +27,7 @@ GP_PROBE_STORE, GP_PROBE_FMA, GP_PROBE_RCP, GP_PROBE_STORE_VIEW = 0, 1, 2, 3
 EXPORTS = ("gp_create", "gp_destroy", "gp_set_option", "gp_scene_upload", "gp_agents_update",
            "gp_cameras_set", "gp_render_batch", "gp_render_batch_host", "gp_stats", "gp_kernel_time",
            "gp_launch_count", "gp_camera_rig_set", "gp_statics_from_polylines", "gp_statics_update",
-           "gp_dynamics_step", "gp_observe_vec", "gp_probe", "gp_reserve", "gp_error_string")
+           "gp_dynamics_step", "gp_observe_vec", "gp_probe", "gp_reserve", "gp_render_static", "gp_error_string")
 
 
 class SceneDesc(ctypes.Structure):
@@ -87,6 +89,7 @@ def lib():
         L.gp_probe.argtypes = [vp, ci, ctypes.c_size_t, ci, vp, vp, vp, vp, vp, ctypes.POINTER(ctypes.c_double),
                                ctypes.POINTER(ctypes.c_double)]
         L.gp_reserve.argtypes = [vp, ci, ci, ci]
+        L.gp_render_static.argtypes = [ci, ctypes.POINTER(SceneDesc), vp, vp, ci, ci, cf, vp, vp, vp, vp, vp]
         L.gp_error_string.argtypes = [ci]
         L.gp_error_string.restype = ctypes.c_char_p
         for name in EXPORTS[:-1]:
@@ -107,6 +110,32 @@ def _stream(device):
 
 def _dptr(t):
     return None if t is None else ctypes.c_void_p(t.data_ptr())
+
+
+def render_static(d_prims, agents_per_world, H, W, fov_rad, d_class, d_instance, d_depth, d_rgb=None, d_pitch_cs=None,
+                  cam_height=1.6, t_max=100.0, light=(0.48, 0.36, 0.8), ambient=0.25, palette=DEFAULT_PALETTE, device=0):
+    """gp_render_static: render every view of a scene that already sits in device memory without the library allocating
+    anything - for processes in which the training framework holds all of HBM, or whose loop cannot take the stall of a
+    cudaMalloc.  No Renderer is needed.  The intermediates live in a fixed 9.1 MiB array inside libgp.so, which limits the
+    scene (GP_STATIC_MAX_VIEWS / _PRIMS / _ENTRIES; GpError with code GP_ERR_LIMIT beyond them) and is shared by all calls
+    on a device: keep them on one stream, or order them, so that they never overlap on the GPU.  The first call on a device
+    does a one-off set-up; make it before any stream capture.
+
+    d_prims: CUDA uint8 tensor [Wn][P][48] of gp_prim records, the agents first in each world; d_pitch_cs: CUDA float32
+    [Wn][A][2] or None (pitch 0); outputs as for Renderer.render_batch with one front camera per agent."""
+    assert d_prims.dim() == 3 and d_prims.shape[2] == 48 and d_prims.is_contiguous()
+    d = SceneDesc()
+    d.n_worlds, d.agents_per_world = int(d_prims.shape[0]), int(agents_per_world)
+    d.quads_per_world = int(d_prims.shape[1]) - int(agents_per_world)
+    d.cam_height, d.t_max, d.ambient = cam_height, t_max, ambient
+    for i in range(3):
+        d.light[i] = light[i]
+    for c in range(min(8, len(palette))):
+        for ch in range(3):
+            d.palette[c][ch] = int(palette[c][ch])
+    _check(lib().gp_render_static(int(device), ctypes.byref(d), _dptr(d_prims), _dptr(d_pitch_cs), int(H), int(W),
+                                  float(fov_rad), _dptr(d_class), _dptr(d_instance), _dptr(d_depth), _dptr(d_rgb),
+                                  _stream(device)))
 
 
 class Renderer:
