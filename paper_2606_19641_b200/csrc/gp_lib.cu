@@ -630,6 +630,11 @@ static int render_device(gp_ctx *c, int world_begin, int n_worlds, int H, int W,
     }
     int rc = ensure_scratch(c, views);
     if (rc != GP_OK) return rc;
+    // Capped lists: the overflow flags are cleared here, BEFORE the fork below, so that the culls on the side stream (which
+    // wait only for the fork event) are ordered behind the clear; issued later on `stream` it could wipe a flag a side-stream
+    // cull had already set, and that view would keep its background-only image
+    const bool capped = c->scratch_cap < sc.P;                         // lists may overflow: flag + brute-force repair pass
+    if (capped) CK(cudaMemsetAsync(c->d_ovf, 0, views, stream));
 
     // ---- pipeline over world chunks: the cull of chunk i + 1 runs on a library-owned high-priority stream while chunk i
     // renders on the caller's stream (the cull is bound by instruction issue and latency, the render by HBM stores,
@@ -666,7 +671,6 @@ static int render_device(gp_ctx *c, int world_begin, int n_worlds, int H, int W,
     cargs.inv_th = 1.0f / th; cargs.inv_tv = 1.0f / tv; cargs.halfW = 0.5f * (float)W; cargs.halfH = 0.5f * (float)H;
     cargs.far_lim = sc.t_max * (1.0f + 1e-6f);
     cargs.cap = c->scratch_cap; cargs.stats = stats;
-    const bool capped = c->scratch_cap < sc.P;                         // lists may overflow: flag + brute-force repair pass
     auto launch_cull = [&](int ci, cudaStream_t st) -> int {
         const int w0 = ci * wpc, nw = std::min(wpc, n_worlds - w0);
         const size_t v0 = (size_t)w0 * vpw;
@@ -725,7 +729,6 @@ static int render_device(gp_ctx *c, int world_begin, int n_worlds, int H, int W,
         ra.magic_vpw = (uint32_t)(((1ull << (31 + L)) + (unsigned)vpw - 1) / (unsigned)vpw);
     }
     const size_t HW = (size_t)H * W;
-    if (capped) CK(cudaMemsetAsync(c->d_ovf, 0, views, stream));
     rc = launch_cull(0, stream);                                       // chunk 0: nothing to overlap with yet
     if (rc != GP_OK) return rc;
     for (int ci = 1; ci < n_chunks; ++ci) {                            // the other culls run ahead on the side stream
