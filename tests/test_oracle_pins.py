@@ -433,3 +433,63 @@ def test_u10_ray_through_a_vertical_box_edge_takes_the_x_face():
     y_face = shade(PAL[VEH], (0.48 - 0.36) * float(c))
     assert x_face != y_face
     assert tuple(int(v) for v in r["rgb"][:, 0, 0]) == x_face
+
+
+# ---------------------------------------------------------------- far plane on primitive hits (reading U2)
+def test_far_plane_on_a_box_is_inclusive_and_cuts_the_whole_face():
+    # CF1's box: its near face is the plane 10 m ahead, so every pixel on it has planar depth exactly 10.0f.
+    # t_max = 10 keeps the face (C5: hit iff t_n <= t_max, inclusive); t_max = 9.99 removes it, and since rows 16-18 meet
+    # the ground at 51.2 / 17.07 / 10.24 m - all beyond either t_max - those six pixels are then sky, like the rest.
+    world = stack(ego_at_origin(), make_prim(12, 0, .75, 2, .9, .75, 1, 0, inst=1))
+    hit = np.zeros((32, 32), bool)
+    hit[16:19, 15:17] = True
+    on = oracle.render_view(world, 0, 32, 32, params=oracle.make_params(t_max=10.0))
+    assert ((on["cls"] == VEH) == hit).all() and (on["depth"][hit] == np.float32(10.0)).all() and (on["inst"][hit] == 1).all()
+    off = oracle.render_view(world, 0, 32, 32, params=oracle.make_params(t_max=9.99))
+    assert (off["cls"][hit] == SKY).all() and (off["depth"][hit] == 0.0).all() and (off["inst"] == -1).all()
+    assert not (off["cls"] == VEH).any()
+    # a face partly beyond the far plane: the box of test_cf1_box_left_and_right_columns shows its near face (depth 10,
+    # columns 10-12) and its inner side face (column 13, depth 13.44); t_max = 11 lies between them, so the near face stays
+    # and column 13 falls back to ground (row 18 would meet it at 10.24 m) or sky
+    left = stack(ego_at_origin(), make_prim(12, 3.0, .75, 2, .9, .75, inst=1))
+    mid = oracle.render_view(left, 0, 32, 32, params=oracle.make_params(t_max=11.0))
+    assert sorted(set(np.nonzero(mid["cls"] == VEH)[1].tolist())) == [10, 11, 12]
+    assert (mid["depth"][mid["cls"] == VEH] == np.float32(10.0)).all()
+    assert mid["cls"][16, 13] == SKY and mid["cls"][17, 13] == SKY and mid["cls"][18, 13] == GROUND
+
+
+def test_i6_tall_box_beyond_the_far_plane_covers_pixel_centres_and_stays_invisible():
+    # A 10 x 6 m wall whose near face is 118 m ahead spans heights 0..6 m: v = (z - 1.6) / 118 in [-0.0136, 0.0373] and
+    # s in +-0.0424.  At 48 x 64 (tv = 0.75) row 23 has v = +0.015625 and columns 31, 32 have s = -+0.015625: two pixel
+    # centres lie on the wall.  With t_max = 100 it is out of range: they are sky and nothing changes; with t_max = 120 they
+    # are the wall at planar depth exactly 118.
+    ego, wall = ego_at_origin(), make_prim(120, 0, 3.0, 2, 5, 3.0, inst=7)
+    base = oracle.render_view(stack(ego), 0, 48, 64)
+    far = oracle.render_view(stack(ego, wall), 0, 48, 64)
+    for k in ("cls", "inst", "depth", "rgb"):
+        assert (base[k] == far[k]).all()
+    near = oracle.render_view(stack(ego, wall), 0, 48, 64, params=oracle.make_params(t_max=120.0))
+    on = np.zeros((48, 64), bool)
+    on[23, 31:33] = True
+    assert ((near["inst"] == 7) == on).all()
+    assert (near["depth"][on] == np.float32(118.0)).all() and (near["cls"][on] == VEH).all()
+
+
+def test_flat_quad_seen_from_below_is_lit_as_from_above():
+    # C8: a flat quad is shaded with its +z normal whichever side the ray comes from (sigma = +1 for h.z == 0).  A 6 x 6 m
+    # marking 3 m above the ground, centred 8 m ahead of a camera at 1.6 m: rays with d.z > 0 meet it from below at
+    # t = 1.4 / v.  n.L = 0.8 -> s8 = int((0.25 + 0.75 * 0.8) * 256) = 217 -> 240 * 217 >> 8 = 203 per channel.
+    quad = make_prim(8, 0, 3.0, 3, 3, 0, cls=MARK, inst=5)
+    r = oracle.render_view(stack(ego_at_origin(), quad), 0, 32, 32)
+    got = r["inst"] == 5
+    v = rows_v(32, 32)[:, None] * np.ones((1, 32))
+    s = cols_s(32)[None, :] * np.ones((32, 1))
+    with np.errstate(divide="ignore"):
+        t = np.where(v > 0, 1.4 / np.where(v > 0, v, 1.0), np.inf)
+    want = (t >= 5) & (t <= 11) & (np.abs(s * t) <= 3)
+    assert want.sum() >= 20 and (got == want).all()
+    assert np.allclose(r["depth"][got], t[got], rtol=1e-6)
+    assert shade(PAL[MARK], 0.8) == (203, 203, 203)
+    for ch in range(3):
+        assert (r["rgb"][ch][got] == 203).all()
+    assert (r["cls"][got] == MARK).all()

@@ -252,3 +252,49 @@ def test_random_scenes_against_an_independent_fp64_argsort(seed):
                     else:
                         assert feat[r, 2] == 2 * prims[w]["hx"][j] and np.allclose(feat[r, 3:5], (dc, ds), atol=1e-6)
                         assert feat[r, 5] == prims[w]["cls"][j] and feat[r, 6] == 1 and feat[r, 7] == 0
+
+
+# ------------------------------------------------------------------------------------------------ update order D3-D5
+# PAPER.md:335 gives no update order (it defers to [16]); DESIGN.md "Dynamics contract" reads it as: accelerations, then
+# speed, then the steering demand from the NEW speed and NEW lateral acceleration, then the heading from the NEW speed and
+# NEW angle, then the position from the NEW speed and NEW heading.  One-step closed forms that tell each choice from "old":
+def test_d5_position_uses_the_new_heading():
+    # heading 0, speed 10, angle d0 held (a_lat demands exactly d0, no jerks): psi1 = v tan(d0) / L dt, and the step is
+    # taken along psi1 - so y1 = v sin(psi1) dt is not 0, as it would be along the old heading
+    L, v, d0, dt = 0.6 * 2 * 2.0, 10.0, 0.2, 0.1
+    par = oracle.make_dyn_params(dt=dt, a_lat_max=20.0, v_max=30.0)
+    st, ps = fresh(v=v, a_lat=v * v * math.tan(d0) / L, steer=d0)
+    s1, p1 = oracle.dynamics_step(par, [act(0.0, 0.0)], [2.0], st, ps)
+    psi1 = v * math.tan(d0) / L * dt
+    assert abs(s1[0, 3] - d0) < 1e-6 and abs(s1[0, 4] - psi1) < 1e-6
+    assert abs(p1[0, 1] - v * math.sin(psi1) * dt) < 1e-6 and p1[0, 1] > 0.08
+    assert abs(p1[0, 0] - v * math.cos(psi1) * dt) < 1e-6
+
+
+def test_d4_heading_uses_the_new_speed():
+    # angle frozen by a zero steering rate, longitudinal acceleration 4 held: psi1 = v' tan(d0) / L dt with v' = v + a_lon dt
+    # (with the old speed it would be 3.4e-3 rad less); the position moves with v' as well
+    L, v, d0, dt, a_lon = 0.6 * 2 * 2.0, 10.0, 0.2, 0.1, 4.0
+    par = oracle.make_dyn_params(dt=dt, steer_rate_max=0.0, v_max=30.0)
+    st, ps = fresh(v=v, a_lon=a_lon, steer=d0)
+    s1, p1 = oracle.dynamics_step(par, [act(0.0, 0.0)], [2.0], st, ps)
+    v1 = v + a_lon * dt
+    psi1 = v1 * math.tan(d0) / L * dt
+    assert abs(s1[0, 0] - v1) < 1e-5 and s1[0, 3] == np.float32(d0)
+    assert abs(s1[0, 4] - psi1) < 1e-6 and abs(psi1 - v * math.tan(d0) / L * dt) > 3e-3
+    assert abs(p1[0, 0] - v1 * math.cos(psi1) * dt) < 1e-6 and abs(p1[0, 1] - v1 * math.sin(psi1) * dt) < 1e-6
+
+
+def test_d3_steering_demand_uses_the_new_speed_and_lateral_acceleration():
+    # demand neither rate- nor magnitude-limited: d1 = atan(L a_lat' / v'^2) with a_lat' = a_lat + j_lat dt and
+    # v' = v + a_lon dt; and since tan(d1) / L = a_lat' / v'^2, the heading advances by exactly a_lat' / v' dt (yaw rate =
+    # lateral acceleration / speed, D4 with the new angle)
+    L, v, dt, a_lon, a_lat = 0.6 * 2 * 2.0, 10.0, 0.1, 4.0, 2.0
+    par = oracle.make_dyn_params(dt=dt, steer_rate_max=100.0, steer_max=1.0, v_max=30.0, a_lat_max=10.0)
+    st, ps = fresh(v=v, a_lon=a_lon, a_lat=a_lat)
+    s1, _ = oracle.dynamics_step(par, [act(0.0, 4.0)], [2.0], st, ps)
+    v1, al1 = v + a_lon * dt, a_lat + 4.0 * dt
+    d1 = math.atan(L * al1 / (v1 * v1))
+    assert abs(s1[0, 2] - al1) < 1e-6 and abs(s1[0, 3] - d1) < 1e-6
+    assert abs(d1 - math.atan(L * al1 / (v * v))) > 3e-3 and abs(d1 - math.atan(L * a_lat / (v1 * v1))) > 3e-3
+    assert abs(s1[0, 4] - al1 / v1 * dt) < 1e-6

@@ -117,3 +117,34 @@ def test_spheres_fp32_quadratic_vs_fp64_closest_approach(seed):
         assert np.allclose(a["depth"][ok], b["depth"][ok], rtol=1e-5, atol=2e-5)
     sph = np.isin(a["inst"], np.arange(20, 30))
     assert bad <= 3, (bad, tot)
+
+
+def test_far_plane_on_a_sphere_is_inclusive():
+    # A sphere of radius 2 centred 12 m ahead at camera height: every surface point has x >= 10, and planar depth IS x, so
+    # the one ray that enters at exactly 10.0 is the central one (33 x 33: pixel (16, 16) has s = v = 0; A = 1, B = -12,
+    # t_ca = 12, half chord 2 -> t_n = 10 exactly in fp32).  t_max = 10 keeps that single pixel (C5s: t_n <= t_max,
+    # inclusive), t_max = 9.99 removes the sphere altogether.  With t_max = 10.5 the drawn part is the cap x <= 10.5,
+    # checked against the fp64 quadratic per pixel.
+    world = stack(ego_at_origin(), make_sphere(12, 0, 1.6, 2.0, inst=4))
+    on = oracle.render_view(world, 0, 33, 33, params=oracle.make_params(t_max=10.0))
+    assert (on["inst"] == 4).sum() == 1 and on["inst"][16, 16] == 4 and on["depth"][16, 16] == np.float32(10.0)
+    off = oracle.render_view(world, 0, 33, 33, params=oracle.make_params(t_max=9.99))
+    assert not (off["inst"] == 4).any() and off["cls"][16, 16] == 0 and off["depth"][16, 16] == 0.0
+    H = W = 65
+    cap = oracle.render_view(world, 0, H, W, params=oracle.make_params(t_max=10.5))
+    i, j = np.mgrid[0:H, 0:W].astype(np.float64)
+    s = (j + 0.5) * 2.0 / W - 1.0
+    v = 1.0 - (i + 0.5) * 2.0 / H
+    d = np.stack([np.ones_like(s), -s, v], axis=-1)                    # camera at (0, 0, 1.6) heading +x: right = -y
+    e = np.array([-12.0, 0.0, 0.0])
+    A = (d * d).sum(-1); B = (d * e).sum(-1); C = 144.0 - 4.0
+    disc = B * B - A * C
+    with np.errstate(invalid="ignore"):
+        t = np.where(disc >= 0, (-B - np.sqrt(np.where(disc >= 0, disc, 0.0))) / A, np.inf)
+    sure_in = t <= 10.5 - 1e-4
+    sure_out = t >= 10.5 + 1e-4
+    got = cap["inst"] == 4
+    assert sure_in.sum() > 20 and got[sure_in].all() and not got[sure_out].any()
+    assert (cap["depth"][got] <= np.float32(10.5)).all()
+    whole = oracle.render_view(world, 0, H, W)
+    assert ((whole["inst"] == 4) & ~got).sum() > 20                     # the rim of the disc lies beyond 10.5 m: cut away
