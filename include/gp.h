@@ -48,15 +48,20 @@ enum {
     GP_OPT_STATS = 2,       /* 1: count executed ray/primitive tests and listed pairs         */
     GP_OPT_TIMING = 3,      /* n > 0: bracket every n-th launch of each kernel with CUDA events
                                (gp_kernel_time); 0: off                                         */
-    GP_OPT_STAGE_CAP = 4,   /* list entries per view staged in shared memory (>= 1; 0 = automatic: 128, or 64 for
-                               images of up to 64 x 64); longer lists read their tail from global memory */
+    GP_OPT_STAGE_CAP = 4,   /* list entries per view staged in shared memory (>= 1); longer lists read their tail from
+                               global memory.  0 = automatic, never more than the primitives per world.  Ray variant:
+                               48 for images of up to 1024 pixels (32 x 32), 64 up to 64 x 64, else 128 - except that a
+                               crowded world (>= 400 primitives, gather mode, 4-warp CTAs) gives up staged entries, down
+                               to 80, when that lets 8 CTAs share an SM instead of 7.  Raster variant: always 128 */
     GP_OPT_STRIP_PX = 5,    /* target pixels per warp strip of the render pass; 0 = automatic   */
     GP_OPT_GATHER = 6,      /* how a strip works off its list: 1 gather the overlapping entries first, one lane
                                per (flat quad, row); 0 entry by entry; -1 (default) chosen from the image size
                                and the primitives per world                                        */
     GP_OPT_VARIANT = 8,     /* render pass: GP_VARIANT_RAY (pixel-major strips), GP_VARIANT_RASTER (primitive-major
-                               tiles with a depth buffer, PAPER.md:62 / :319) or -1 (default): chosen per launch
-                               shape from measurements.  Results are bit-identical.   */
+                               tiles with a depth buffer, PAPER.md:62 / :319) or -1 (default) = the ray variant for
+                               every shape: the raster variant measured 7-41 % slower on all six shapes tried
+                               (profiles/r02_raster_vs_ray.md) and is kept as the selectable alternative.
+                               Results are bit-identical.                                            */
     GP_OPT_TILE_PX = 9,     /* raster variant: target pixels per tile; 0 = automatic                   */
     GP_OPT_PIPELINE = 10,   /* n >= 1 world chunks per gp_render_batch; with n > 1 the culls of chunks 1.. run on a
                                library-owned high-priority stream concurrently with the renders of earlier chunks.
@@ -275,7 +280,7 @@ typedef struct {
     float a_lon_max;        /* |longitudinal acceleration| limit, m/s^2                                */
     float a_lat_max;        /* |lateral acceleration| limit, m/s^2                                     */
     float v_max;            /* speed limit, m/s: speed is clipped to [0, v_max] (no reversing)         */
-    float steer_max;        /* |steering angle| limit, rad                                             */
+    float steer_max;        /* |steering angle| limit, rad; below pi/2 (GP_ERR_ARG otherwise)          */
     float steer_rate_max;   /* |steering rate| limit, rad/s                                            */
     float v_eps;            /* the curvature demand a_lat / v^2 uses max(v, v_eps), m/s (> 0)          */
     float extent;           /* > 0: positions wrap onto the torus [-extent/2, extent/2); 0: no wrap    */
@@ -284,13 +289,15 @@ typedef struct {
 /* One simulation step of every agent, on the device (DESIGN.md "Dynamics contract" D1-D6), fused with
  * the pose update a0 of gp_agents_update:
  *   d_action DEVICE int32 [Wn][A]: one of the twelve actions, = 3 * i_lon + i_lat with longitudinal jerk
- *            {-15, -4, 0, 4}[i_lon] and lateral jerk {-4, 0, 4}[i_lat] m/s^3; other values leave the agent untouched
+ *            {-15, -4, 0, 4}[i_lon] and lateral jerk {-4, 0, 4}[i_lat] m/s^3; other values leave the agent untouched,
+ *            and so does an agent record of zero length (hx == 0: it has no wheelbase)
  *   d_state  DEVICE fp32 [Wn][A][8], in / out: speed v, a_lon, a_lat, steering angle, heading psi in [-pi, pi), 3 unused
  *   d_pose   DEVICE fp32 [Wn][A][4], in / out: (cx, cy, cos psi, sin psi) — the layout gp_agents_update takes
  * Jerks -> accelerations (clipped) -> speed (clipped to [0, v_max]) -> steering angle demanded by a_lat = v^2 kappa with
  * kappa = tan(steer) / L, wheelbase L = 0.6 * vehicle length (2 hx of the agent's record), bounded in rate and
  * magnitude -> heading -> position (new speed and heading; optional torus wrap).  The new poses are also written into
  * the scene (agent records + shading table), so gp_render_batch can follow with no host transfer.
+ * The heading is wrapped into [-pi, pi) however far it turned in the step.
  * fp32 arithmetic with atanf / tanf / sincosf.  Both pointers 16-byte aligned. */
 int gp_dynamics_step(gp_ctx *ctx, const gp_dyn_params *params, const int32_t *d_action, float *d_state,
                      float *d_pose, void *stream);
@@ -320,7 +327,7 @@ int gp_observe_vec(gp_ctx *ctx, const float *d_state, int K, int M, float radius
  *     class plane and the three colour planes, 16-byte stores to the instance and depth planes = 12 B / pixel) over
  *     n_pixels pixels (a multiple of 128) of the caller's DEVICE planes (sized as for gp_render_batch with n_pixels
  *     pixels in all; their content is overwritten).  Result: GB/s.
- *   GP_PROBE_FMA: 8 independent FFMA chains per thread on 148 x 8 CTAs x 256 threads, no memory traffic; the plane
+ *   GP_PROBE_FMA: 8 independent FFMA chains per thread on (SM count) x 8 CTAs x 256 threads, no memory traffic; the plane
  *     pointers and n_pixels are ignored.  Result: TFLOP/s (2 flop per FFMA) at the clock the GPU runs this at.
  *   GP_PROBE_STORE_VIEW: the same store stream with the render pass's CTA -> address mapping: one CTA per view of the
  *     image size of the last gp_render_batch (H * W a multiple of 128; GP_ERR_STATE before any render), n_pixels a
@@ -329,7 +336,8 @@ int gp_observe_vec(gp_ctx *ctx, const float *d_state, int K, int M, float radius
  *   GP_PROBE_RCP: self-check of the render pass's paired reciprocal (C0: 1.0f / x correctly rounded) against
  *     __frcp_rn on all 2^32 bit patterns; the plane pointers and n_pixels are ignored.  Result: the number of bit
  *     patterns whose result differed, summed over the launches (0 = identical).
- * Runs `iters` timed launches after one warm-up; *best = highest rate, *median (may be NULL) = the median. */
+ * Runs `iters` timed launches after one warm-up; *best = highest rate, *median (may be NULL) = the median.
+ * The probes use device words of their own: the counters gp_stats reads are not disturbed. */
 enum { GP_PROBE_STORE = 0, GP_PROBE_FMA = 1, GP_PROBE_RCP = 2, GP_PROBE_STORE_VIEW = 3 };
 int gp_probe(gp_ctx *ctx, int kind, size_t n_pixels, int iters, uint8_t *d_class, int32_t *d_instance, float *d_depth,
              uint8_t *d_rgb, void *stream, double *best, double *median);

@@ -169,10 +169,11 @@ def render_views(world_prims, views, H, W, params=None, pitch_cs=None, rgb=True,
         return list(ex.map(one, views))
 
 
-def dynamics_step(params, action, half_len, state, pose):
+def dynamics_step(params, action, half_len, state, pose, strict=True):
     """One step of the jerk bicycle for n agents (fp64 inside, fp32 in / out).  action int32 [n], half_len fp32 [n],
     state fp32 [n][8] = (v, a_lon, a_lat, steer, psi, -, -, -), pose fp32 [n][4] = (x, y, cos psi, sin psi).
-    Returns (new_state, new_pose); the inputs are not modified."""
+    Returns (new_state, new_pose); the inputs are not modified.  An action outside [0, 12) or a half length <= 0 leaves
+    that agent untouched: ValueError when `strict`, otherwise the result with those agents unchanged."""
     action = np.ascontiguousarray(action, dtype=np.int32).reshape(-1)
     n = action.size
     half_len = np.ascontiguousarray(half_len, dtype=np.float32).reshape(n)
@@ -180,7 +181,7 @@ def dynamics_step(params, action, half_len, state, pose):
     ps = np.array(pose, dtype=np.float32, copy=True).reshape(n, 4)
     rc = lib().orc_dynamics_step(ctypes.byref(params), n, action.ctypes.data, half_len.ctypes.data,
                                  st.ctypes.data, ps.ctypes.data)
-    if rc != 0:
+    if rc != 0 and (strict or rc != -2):
         raise ValueError("orc_dynamics_step: bad arguments (%d)" % rc)
     return st.reshape(np.shape(state)), ps.reshape(np.shape(pose))
 

@@ -58,8 +58,8 @@ static double clipd(double x, double lo, double hi) { return x < lo ? lo : (x > 
 /* One step for n agents.  action[n] in [0, 12): longitudinal jerk index = action / 3, lateral = action % 3.
  * state[n][8] fp32 in/out: v, a_lon, a_lat, steer, psi, 3 unused.  pose[n][4] fp32 in/out: x, y, cos psi, sin psi
  * (the buffer the renderer's pose update consumes).  half_len[n]: half length hx of each agent's box (wheelbase =
- * 0.6 * 2 hx).  Returns 0, or -1 on bad arguments (an action outside [0, 12) leaves that agent untouched and
- * makes the call return -2 after processing the others). */
+ * 0.6 * 2 hx).  Returns 0, or -1 on bad arguments (an action outside [0, 12) or a half length <= 0 leaves that agent
+ * untouched and makes the call return -2 after processing the others). */
 int orc_dynamics_step(const orc_dyn_params *par, int n, const int32_t *action, const float *half_len,
                       float *state, float *pose)
 {
@@ -69,6 +69,7 @@ int orc_dynamics_step(const orc_dyn_params *par, int n, const int32_t *action, c
     for (int i = 0; i < n; ++i) {
         int a = action[i];
         if (a < 0 || a >= 12) { rc = -2; continue; }
+        if (!(half_len[i] > 0.0f)) { rc = -2; continue; }     /* no length, no wheelbase: untouched, like an invalid action */
         float *s = state + (size_t)i * 8, *p = pose + (size_t)i * 4;
         double v = s[0], a_lon = s[1], a_lat = s[2], steer = s[3], psi = s[4];
         double x = p[0], y = p[1];
@@ -88,6 +89,7 @@ int orc_dynamics_step(const orc_dyn_params *par, int n, const int32_t *action, c
         /* D4: heading, wrapped into [-pi, pi) */
         psi = psi + v * (tan(steer) / L) * dt;
         const double PI = 3.14159265358979323846;
+        if (fabs(psi) > 2.0 * PI) psi = remainder(psi, 2.0 * PI);     /* more than a full turn in one step */
         if (psi >= PI) psi -= 2.0 * PI;
         if (psi < -PI) psi += 2.0 * PI;
         /* D5: position with the NEW speed and heading (semi-implicit Euler) */

@@ -24,6 +24,7 @@ __global__ void k_dynamics_step(SceneConst sc, gp_dyn_params par, const int32_t 
     if (a < 0 || a >= 12) return;                                   // invalid action: the agent is left untouched
     const size_t w = i / sc.A, ag = i % sc.A;
     gp_prim *p = &prims[w * sc.P + ag];
+    if (!(p->hx > 0.0f)) return;                                    // no length, no wheelbase (tan / L): left untouched too
     const float4 s0 = state[2 * i], s1 = state[2 * i + 1], ps = pose[i];
     const int il = a / 3, it = a - 3 * il;
     const float jlon = il == 0 ? -15.0f : il == 1 ? -4.0f : il == 2 ? 0.0f : 4.0f;
@@ -41,6 +42,7 @@ __global__ void k_dynamics_step(SceneConst sc, gp_dyn_params par, const int32_t 
     steer = clipf(steer, -par.steer_max, par.steer_max);
     psi = fmaf(v * (tanf(steer) / L), dt, psi);                                          // D4
     const float PI = 3.14159265358979323846f;
+    if (fabsf(psi) > 2.0f * PI) psi = remainderf(psi, 2.0f * PI);                        // more than a turn in one step (exact)
     if (psi >= PI) psi -= 2.0f * PI;
     if (psi < -PI) psi += 2.0f * PI;
     float sn, c;

@@ -38,7 +38,8 @@ struct gp_ctx {
     ViewHdr *d_hdr = nullptr; EntryGeo *d_geo = nullptr; EntryAux *d_aux = nullptr;
     uint8_t *d_ovf = nullptr;                                    // per view: its list did not fit GP_OPT_LIST_CAP
     size_t scratch_views = 0; int scratch_cap = 0;
-    unsigned long long *d_stats = nullptr;
+    unsigned long long *d_stats = nullptr;                      // [0..1] GP_OPT_STATS counters, [2..3] scratch of gp_probe
+    int n_sms = 148;
     int opt_path = GP_PATH_FAST, opt_stats = 0, opt_timing = 0, opt_stage_cap = 0, opt_strip_px = 0, opt_gather = -1, opt_spheres = -1;
     int opt_variant = -1, opt_tile_px = 0, opt_pipeline = 1, opt_list_cap = 0;
     cudaStream_t aux_stream = nullptr;                           // culls of later chunks run here (render_device)
@@ -136,9 +137,10 @@ extern "C" int gp_create(gp_ctx **out, int cuda_device) {
     c->device = cuda_device;
     c->sc.C = 1;                                                   // default rig: one front camera
     c->sc.rig[0] = make_float4(1.0f, 0.0f, 1.0f, 0.0f);
-    cudaError_t e = cudaMalloc(&c->d_stats, 2 * sizeof(unsigned long long));
+    c->n_sms = prop.multiProcessorCount;
+    cudaError_t e = cudaMalloc(&c->d_stats, 4 * sizeof(unsigned long long));
     if (e != cudaSuccess) { delete c; return cuda_fail(e, "cudaMalloc(stats)"); }
-    cudaMemset(c->d_stats, 0, 2 * sizeof(unsigned long long));
+    cudaMemset(c->d_stats, 0, 4 * sizeof(unsigned long long));
     *out = c;
     return GP_OK;
 }
@@ -298,6 +300,7 @@ extern "C" int gp_dynamics_step(gp_ctx *c, const gp_dyn_params *par, const int32
     if (!(par->dt > 0.0f) || !(par->a_lon_max >= 0.0f) || !(par->a_lat_max >= 0.0f) || !(par->v_max >= 0.0f) ||
         !(par->steer_max >= 0.0f) || !(par->steer_rate_max >= 0.0f) || !(par->v_eps > 0.0f) || !(par->extent >= 0.0f))
         return GP_ERR_ARG;
+    if (!(par->steer_max < 1.5707f)) return GP_ERR_ARG;             // tan(steer) must stay finite
     if (!aligned16(d_state) || !aligned16(d_pose)) return GP_ERR_ALIGN;
     GP_ON_DEVICE(c);
     const size_t n = (size_t)c->sc.Wn * c->sc.A;
@@ -876,7 +879,10 @@ extern "C" int gp_probe(gp_ctx *c, int kind, size_t n_pixels, int iters, uint8_t
     GP_ON_DEVICE(c);
     cudaStream_t stream = static_cast<cudaStream_t>(stream_);
     cudaEvent_t e0, e1;
-    CK(cudaEventCreate(&e0)); CK(cudaEventCreate(&e1));
+    CK(cudaEventCreate(&e0));
+    { cudaError_t e = cudaEventCreate(&e1); if (e != cudaSuccess) { cudaEventDestroy(e0); return cuda_fail(e, "cudaEventCreate"); } }
+    unsigned long long *d_probe = c->d_stats + 2;               // the probes' own words: the GP_OPT_STATS counters stay intact
+    const unsigned probe_grid = (unsigned)c->n_sms * 8;
     std::vector<double> rate;
     int rc = GP_OK;
     for (int it = 0; it < iters + 1 && rc == GP_OK; ++it) {                 // the first launch is a warm-up
@@ -900,11 +906,14 @@ extern "C" int gp_probe(gp_ctx *c, int kind, size_t n_pixels, int iters, uint8_t
             units = (double)n_pixels * 12.0 / 1e9;                              // GB
         } else if (kind == GP_PROBE_FMA) {
             const int reps = 4096;
-            k_probe_fma<<<148 * 8, 256, 0, stream>>>(reps, 1.0f + (float)it, reinterpret_cast<float *>(c->d_stats));
-            units = 2.0 * 148.0 * 8 * 256 * (double)reps * 16 * 8 / 1e12;       // TFLOP
+            k_probe_fma<<<probe_grid, 256, 0, stream>>>(reps, 1.0f + (float)it, reinterpret_cast<float *>(d_probe));
+            units = 2.0 * (double)probe_grid * 256 * (double)reps * 16 * 8 / 1e12;   // TFLOP
         } else if (kind == GP_PROBE_RCP) {
-            if (it == 0) CK(cudaMemsetAsync(c->d_stats, 0, sizeof(unsigned long long), stream));   // count over all launches
-            k_probe_rcp<<<148 * 8, 256, 0, stream>>>(c->d_stats);
+            if (it == 0) {                                                                          // count over all launches
+                cudaError_t e = cudaMemsetAsync(d_probe, 0, sizeof(unsigned long long), stream);
+                if (e != cudaSuccess) { rc = cuda_fail(e, "cudaMemsetAsync(probe)"); break; }
+            }
+            k_probe_rcp<<<probe_grid, 256, 0, stream>>>(d_probe);
             units = 0.0;
         } else { rc = GP_ERR_ARG; break; }
         c->launches += 1;
@@ -918,8 +927,8 @@ extern "C" int gp_probe(gp_ctx *c, int kind, size_t n_pixels, int iters, uint8_t
     if (rc != GP_OK) return rc;
     if (kind == GP_PROBE_RCP) {                                                 // result = mismatching bit patterns
         unsigned long long bad = 0;
-        CK(cudaMemcpy(&bad, c->d_stats, sizeof bad, cudaMemcpyDeviceToHost));
-        CK(cudaMemset(c->d_stats, 0, sizeof bad));
+        CK(cudaMemcpy(&bad, d_probe, sizeof bad, cudaMemcpyDeviceToHost));
+        CK(cudaMemset(d_probe, 0, sizeof bad));
         *best = (double)bad;
         if (median) *median = (double)bad;
         return GP_OK;

@@ -135,6 +135,47 @@ def test_dynamics_limits_and_invalid_actions(torch_cuda):
     r.close()
 
 
+def test_dynamics_full_turns_zero_length_and_steer_limit(torch_cuda):
+    """more than a full turn in one step still lands in [-pi, pi); an agent record of zero length (no wheelbase)
+    is left untouched instead of turning NaN; steer_max >= pi/2 is refused."""
+    torch = torch_cuda
+    from paper_2606_19641_b200 import GpError, gp
+    cfg = gs.config("small", n_worlds=4)
+    agents, quads = gs.gen_world_prims(cfg)
+    agents = agents.copy()
+    agents["hx"][1, :] = 0.25                                    # L = 0.3 m: 17 rad per step at full lock
+    agents["hx"][2, ::2] = 0.0                                   # zero length
+    r = renderer_for(cfg, agents, quads)
+    par = dict(PAR, steer_max=1.3, steer_rate_max=0.0, v_max=30.0)
+    st, pose = initial_state(cfg, agents, 21)
+    st[1, :, 0] = 20.0
+    st[1, :, 3] = np.where(np.arange(cfg.agents) % 2, 1.2, -1.2)
+    action = np.full(agents.shape, 7, np.int32)                  # zero jerks
+    d_st, d_pose = torch.from_numpy(st).cuda(), torch.from_numpy(pose).cuda()
+    r.dynamics_step(par, torch.from_numpy(action).cuda(), d_st, d_pose)
+    o_st, o_pose = oracle.dynamics_step(oracle.make_dyn_params(**par), action, agents["hx"].reshape(-1), st.reshape(-1, 8),
+                                        pose.reshape(-1, 4), strict=False)
+    g_st, g_pose = d_st.cpu().numpy(), d_pose.cpu().numpy()
+    o_st, o_pose = o_st.reshape(st.shape), o_pose.reshape(pose.shape)
+    assert np.isfinite(g_st).all() and np.isfinite(g_pose).all()
+    assert np.array_equal(g_st[2, ::2], st[2, ::2]) and np.array_equal(g_pose[2, ::2], pose[2, ::2])
+    assert np.array_equal(o_st[2, ::2], st[2, ::2])
+    assert ((g_st[..., 4] >= -math.pi) & (g_st[..., 4] < math.pi + 1e-6)).all()
+    turned = np.abs(20.0 * math.tan(1.2) / 0.3 * 0.1)
+    assert turned > 4 * math.pi
+    # a heading of 17 rad before the wrap carries ~8 ulp(17) = 1.5e-5 of fp32 error: the tolerance scales with it
+    assert ang_diff(g_st[..., 4], o_st[..., 4]).max() <= 3e-5
+    assert np.abs(g_pose[..., 2:].astype(np.float64) - o_pose[..., 2:]).max() <= 3e-5
+    assert np.abs(g_pose[..., :2].astype(np.float64) - o_pose[..., :2]).max() <= 1e-4
+    keep = np.ones(agents.shape, bool); keep[1] = False
+    check_dyn(g_st[keep], g_pose[keep], o_st[keep], o_pose[keep], 0.0)      # everyone else at the usual tolerance
+    for bad in (math.pi / 2, 2.0):
+        with pytest.raises(GpError) as ei:
+            r.dynamics_step(dict(PAR, steer_max=bad), torch.from_numpy(action).cuda(), d_st, d_pose)
+        assert ei.value.code == gp.GP_ERR_ARG
+    r.close()
+
+
 def test_dynamics_feeds_the_renderer_without_the_host(torch_cuda):
     # gp_dynamics_step also performs the pose update a0: rendering right after it must equal, bit for bit, rendering
     # after an explicit gp_agents_update with the pose buffer it produced (render parity itself: test_gpu_parity.py)

@@ -298,3 +298,30 @@ def test_d3_steering_demand_uses_the_new_speed_and_lateral_acceleration():
     assert abs(s1[0, 2] - al1) < 1e-6 and abs(s1[0, 3] - d1) < 1e-6
     assert abs(d1 - math.atan(L * al1 / (v * v))) > 3e-3 and abs(d1 - math.atan(L * a_lat / (v1 * v1))) > 3e-3
     assert abs(s1[0, 4] - al1 / v1 * dt) < 1e-6
+
+
+def test_heading_wrap_after_more_than_a_full_turn_in_one_step():
+    # D4 wraps the heading into [-pi, pi); a short vehicle at full lock turns several times in one step:
+    # v = 20, angle 1.2 frozen, L = 0.6 * 2 * 0.25 = 0.3 -> 20 tan(1.2) / 0.3 * 0.1 = 17.15 rad = 2.73 turns.  ADVICE r2.
+    for psi0, sgn in ((0.3, 1.0), (-2.0, -1.0)):
+        par = oracle.make_dyn_params(dt=0.1, steer_max=1.3, steer_rate_max=0.0, v_max=30.0)
+        st, ps = fresh(v=20.0, steer=sgn * 1.2, psi=psi0)
+        s1, p1 = oracle.dynamics_step(par, [act(0.0, 0.0)], [0.25], st, ps)
+        turned = psi0 + sgn * 20.0 * math.tan(1.2) / 0.3 * 0.1
+        assert abs(turned) > 2 * math.pi + 1.0
+        want = (turned + math.pi) % (2 * math.pi) - math.pi
+        assert -math.pi <= s1[0, 4] < math.pi and abs(s1[0, 4] - want) < 1e-5
+        assert abs(p1[0, 2] - math.cos(turned)) < 1e-5 and abs(p1[0, 3] - math.sin(turned)) < 1e-5
+        assert abs(p1[0, 0] - 2.0 * math.cos(turned)) < 1e-5 and abs(p1[0, 1] - 2.0 * math.sin(turned)) < 1e-5
+
+
+def test_zero_length_agent_is_left_untouched():
+    # the wheelbase is 0.6 * length: an agent record of zero length has no curvature tan(steer) / L, so the step skips it
+    # like an agent with an invalid action instead of writing inf / NaN into its state
+    par = oracle.make_dyn_params()
+    st, ps = fresh(n=2, v=5.0, steer=0.1, a_lat=1.0)
+    with pytest.raises(ValueError):
+        oracle.dynamics_step(par, [act(4.0, 4.0)] * 2, [2.0, 0.0], st, ps)
+    s1, p1 = oracle.dynamics_step(par, [act(4.0, 4.0)] * 2, [2.0, 0.0], st, ps, strict=False)
+    assert np.array_equal(s1[1], st[1]) and np.array_equal(p1[1], ps[1])
+    assert s1[0, 0] > 5.0 and p1[0, 0] > 0.4 and np.isfinite(s1).all() and np.isfinite(p1).all()
