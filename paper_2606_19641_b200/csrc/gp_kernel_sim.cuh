@@ -93,13 +93,15 @@ __device__ __forceinline__ void obs_select(unsigned long long *keys, int n, int 
     }
 }
 
-// The same selection for n <= 32 N candidates with the keys in REGISTERS: every lane holds N keys (candidates lane,
-// lane + 32, ...), sorts them once with a compile-time bitonic network, and the rounds become a 32-way merge of the
-// lanes' sorted runs: warp minimum of the heads by two 32-bit warp reductions (REDUX: high word = d2 bits, then the
-// index among the lanes that tie on it), the winning lane pops its head.  ~25 instructions per round instead of a
-// shared-memory scan of all keys: 2.2 x fewer instructions at K = 16, M = 32 over 64 agents / 200 segments.
+// The same selection for n <= 32 N candidates: every lane takes N keys (candidates lane, lane + 32, ...) into registers,
+// sorts them once with a compile-time bitonic network and writes its sorted run back to its own slots of the warp's key
+// array (which the host sizes to 32 (N + 1) slots: obs_key_slots).  The rounds are then a 32-way merge of the lanes' runs that
+// keeps only each run's head in registers: warp minimum of the heads' d2 bits, then of the indices among the lanes that
+// hold it (two REDUX; O1: lowest index first), and the one winning lane records its index and takes its next key from
+// shared memory.  ~15 instructions per round, no branch; round 2 shifted the whole
+// run down through 2 N registers per round instead (30 instructions; ncu: 65 % of the kernel's instructions).
 template <int N>
-__device__ __forceinline__ void obs_merge(const unsigned long long *keys, int n, int rounds, int *sel, int lane) {
+__device__ __forceinline__ void obs_merge(unsigned long long *keys, int n, int rounds, int *sel, int lane) {
     unsigned long long k[N];
 #pragma unroll
     for (int t = 0; t < N; ++t) { const int q = lane + 32 * t; k[t] = q < n ? keys[q] : kObsNone; }
@@ -117,18 +119,38 @@ __device__ __forceinline__ void obs_merge(const unsigned long long *keys, int n,
                     k[i] = sw ? y : x; k[j] = sw ? x : y;
                 }
             }
-    for (int r = 0; r < rounds; ++r) {
-        const uint32_t hi = (uint32_t)(k[0] >> 32), lo = (uint32_t)k[0];
+    // rounds beyond the number of candidates within the radius are padding: count them once instead of testing every round
+    int valid = 0;
+#pragma unroll
+    for (int t = 0; t < N; ++t) valid += (uint32_t)(k[t] >> 32) != 0xffffffffu;      // d2 bits < 0x7f800000: all ones = "none"
+    const int live = min(rounds, (int)__reduce_add_sync(0xffffffffu, (unsigned)valid));
+#pragma unroll
+    for (int t = 1; t < N; ++t) keys[lane + 32 * t] = k[t];                  // the run behind the head, in the lane's own slots
+    keys[lane + 32 * N] = kObsNone;                                          // ... closed by a sentinel (no bound test per round)
+    uint32_t hi = (uint32_t)(k[0] >> 32), lo = (uint32_t)k[0];
+    const unsigned long long *next = keys + lane + 32;                       // the key behind the head
+    uint32_t sel_addr = (uint32_t)__cvta_generic_to_shared(sel);
+    for (int r = 0; r < live; ++r, sel_addr += 4) {
+        // two dependent warp minima, no branch: the smallest d2 among the heads, then the lowest index among the lanes that
+        // hold it (O1; exactly one lane wins).  A ballot + "more than one bit?" test would save the second REDUX in the
+        // common case, but costs a branch and a convergence barrier per round (measured: 24 instructions per round against 15)
         const uint32_t mh = __reduce_min_sync(0xffffffffu, hi);
         const uint32_t ml = __reduce_min_sync(0xffffffffu, hi == mh ? lo : 0xffffffffu);
-        if (lane == 0) sel[r] = mh == 0xffffffffu ? -1 : (int)ml;            // d2 bits < 0x7f800000: 0xffffffff only for "none"
-        if (hi == mh && lo == ml && mh != 0xffffffffu) {                     // the winner pops its head
-#pragma unroll
-            for (int t = 0; t + 1 < N; ++t) k[t] = k[t + 1];
-            k[N - 1] = kObsNone;
-        }
+        const bool win = hi == mh && lo == ml;
+        const unsigned long long nx = *next;                                 // every lane reads; only the winner takes it
+        asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %0, 0;\n\t@p st.shared.u32 [%1], %2;\n\t}"
+                     :: "r"((unsigned)win), "r"(sel_addr), "r"(lo) : "memory");
+        hi = win ? (uint32_t)(nx >> 32) : hi;
+        lo = win ? (uint32_t)nx : lo;
+        next += win ? 32 : 0;
     }
+    for (int q = live + lane; q < rounds; q += 32) sel[q] = -1;
     __syncwarp();
+}
+
+// Slots of the per-warp key array for n candidates (host and device agree): 32 (N + 1) for the register-sorted merge.
+__host__ __device__ inline int obs_key_slots(int n) {
+    return n <= 64 ? 96 : n <= 128 ? 160 : n <= 256 ? 288 : n <= 512 ? 544 : n;      // 32 N run slots + 32 sentinels
 }
 
 __device__ __forceinline__ void obs_pick(unsigned long long *keys, int n, int rounds, int idx_base, int *sel, int lane) {
@@ -140,13 +162,14 @@ __device__ __forceinline__ void obs_pick(unsigned long long *keys, int n, int ro
 }
 
 // Grid: one CTA per (world, group of nwarps agents).  Dynamic shared memory: float4 s_a[P] (x, y, cos, sin),
-// float4 s_b[P] (2 hx, 2 hy, speed | cls, road flag), unsigned long long s_keys[nwarps][max(A, Q)], int s_sel[nwarps][max(K, M)].
+// float4 s_b[P] (2 hx, 2 hy, speed | cls, road flag), unsigned long long s_keys[nwarps][obs_key_slots(max(A, Q))],
+// int s_sel[nwarps][max(K, M)].
 __global__ void __launch_bounds__(kObsWarps * 32)
 k_observe_vec(SceneConst sc, ObsArgs oa, const gp_prim *__restrict__ prims) {
     extern __shared__ __align__(16) unsigned char smem[];
     const int P = sc.P, A = sc.A, Q = sc.Q;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int nmax = max(A, Q), rmax = max(oa.K, oa.M);
+    const int nmax = obs_key_slots(max(A, Q)), rmax = max(oa.K, oa.M);
     float4 *s_a = reinterpret_cast<float4 *>(smem);
     float4 *s_b = s_a + P;
     unsigned long long *s_keys = reinterpret_cast<unsigned long long *>(s_b + P) + (size_t)warp * nmax;

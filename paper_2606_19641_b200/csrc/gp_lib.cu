@@ -327,7 +327,7 @@ extern "C" int gp_observe_vec(gp_ctx *c, const float *d_state, int K, int M, flo
     oa.state = reinterpret_cast<const float4 *>(d_state);
     oa.agent_idx = d_agent_idx; oa.agent_feat = d_agent_feat; oa.road_idx = d_road_idx; oa.road_feat = d_road_feat;
     // agents per CTA: as many warps (<= kObsWarps) as leave the world's records + per-warp key arrays within shared memory
-    const size_t nmax = (size_t)std::max(sc.A, sc.Q), rmax = (size_t)std::max(K, M);
+    const size_t nmax = (size_t)obs_key_slots(std::max(sc.A, sc.Q)), rmax = (size_t)std::max(K, M);
     int nw = std::min(kObsWarps, sc.A);
     size_t smem = 0;
     for (;; --nw) {
