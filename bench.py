@@ -491,6 +491,14 @@ def run_b200(args):
                           "views_per_s": world_size * cfg.views * sim_steps / (sim_ms * 1e-3),
                           "kernels_ms_per_step": {k: v[0] / n_s for k, v in kt.items()},
                           "gpu_launches": int(r.launch_count() - l0),
+                          "roofline_observe": (lambda b, t: {
+                              "bound": "hbm", "kernel": "k_observe_vec", "algorithmic_bytes": b, "avg_launch_ms": t,
+                              "achieved": b / (t * 1e-3) / 1e9, "peak": peaks()[0], "unit": "GB/s", "frac": b / (t * 1e-3) / 1e9 / peaks()[0],
+                              "note": "bytes = Wn P 48 (records) + Wn A 32 (state) read + Wn A (K + M) 36 written; the kernel is bound by "
+                                      "instruction issue, not by HBM (profiles/r03_observe.md): 1528 warp instructions per agent, 75 % of "
+                                      "the issue slots"})(
+                              cfg.n_worlds * cfg.prims * 48 + cfg.n_worlds * cfg.agents * (32 + (K_OBS + M_OBS) * 36),
+                              kt["observe"][0] / n_s),
                           "what": "gp_dynamics_step (12 random actions, dt 0.1 s, torus %g m) + gp_observe_vec (K=%d agents, M=%d road "
                                   "segments, %g m) + gp_render_batch, all on the device" % (cfg.extent, K_OBS, M_OBS, RADIUS),
                           "context": "PAPER.md:8 quotes ~50k agent steps/s on 1 GPU for its simulator with rendering (other hardware, "
