@@ -557,7 +557,7 @@ def run_b200(args):
     # dram bytes of one k_render launch from a COMMITTED ncu --set full capture of this command (not measured live:
     # a run under the profiler is never a bench run); the file names its source captures
     traffic, traffic_source = None, None
-    for tname in ("r02_traffic.txt", "r01_traffic.txt"):
+    for tname in ("r03_traffic.txt", "r02_traffic.txt"):
         tpath = os.path.join(ROOT, "profiles", tname)
         if traffic is None and os.path.exists(tpath) and not args.worlds and not args.hw:
             for line in open(tpath):
